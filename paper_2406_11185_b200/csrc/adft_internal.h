@@ -1,0 +1,33 @@
+// adft_internal.h -- host-side structures shared by the C-ABI translation unit and the class instantiation units.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/adft.h"
+#include "adft_device.cuh"
+
+namespace adft {
+
+constexpr int NPAIRCLASS = 10;     // (la>=lb), la<=3:  pc = la(la+1)/2+lb
+constexpr int NQCLASS = 55;        // X(X+1)/2+Y, X>=Y
+
+inline int pair_class(int la, int lb) { return la * (la + 1) / 2 + lb; }       // requires la >= lb
+inline int quartet_class(int X, int Y) { return X * (X + 1) / 2 + Y; }          // requires X >= Y
+
+// Per-class launchers, filled by the instantiation units (one per generated class).
+struct ClassEntry {
+    void (*launch_jk)(const JKParams &p, cudaStream_t st, bool want_j, bool want_k) = nullptr;
+    void (*launch_schwarz)(const PairTable &t, int pair_base, int prim_base, int n, int K, const double *boys,
+                           double *Qout, cudaStream_t st) = nullptr;
+    int la = 0, lb = 0, lc = 0, ld = 0;
+    int vrr_ops = 0, hrr_ops = 0, nint = 0;   // FP64 instruction counts from the generator
+    const char *impl = "none";                // "straightline" | "table"
+};
+ClassEntry *class_table();                    // [NQCLASS]
+void register_all_classes();                  // defined in generated registry.cu
+
+void set_error(const std::string &msg);
+
+}  // namespace adft

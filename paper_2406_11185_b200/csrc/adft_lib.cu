@@ -1,0 +1,718 @@
+// adft_lib.cu -- the C ABI of include/adft.h: basis ingest (a1), shell-pair table + Schwarz (a2),
+// screening plan (a3), class launches (a4/a5), finalise (a6), stats, FP64 peak microbenchmark.
+#include <algorithm>
+#include <cfloat>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+#include "adft_internal.h"
+
+namespace adft {
+
+static thread_local std::string g_last_error;
+void set_error(const std::string &msg) { g_last_error = msg; }
+
+static ClassEntry g_classes[NQCLASS];
+ClassEntry *class_table() { return g_classes; }
+static bool g_registered = false;
+static void ensure_registered()
+{
+    if (!g_registered) { register_all_classes(); g_registered = true; }
+}
+
+#define CUDA_TRY(expr)                                                                           \
+    do {                                                                                         \
+        cudaError_t e__ = (expr);                                                                \
+        if (e__ != cudaSuccess) {                                                                \
+            set_error(std::string(#expr) + ": " + cudaGetErrorString(e__));                      \
+            return ADFT_ERR_CUDA;                                                                \
+        }                                                                                        \
+    } while (0)
+
+static inline int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+
+// ------------------------------------------------------------------ small kernels
+// (a2) primitive-pair records of one sublist (all pairs share la, lb and K = npa*npb).
+__global__ void pair_prim_kernel(int pair_base, int prim_base, int n, const int32_t *__restrict__ sha,
+                                 const int32_t *__restrict__ shb, const int32_t *__restrict__ sh_atom,
+                                 const int32_t *__restrict__ sh_nprim, const int32_t *__restrict__ sh_off,
+                                 const double *__restrict__ xyz, const double *__restrict__ expo,
+                                 const double *__restrict__ coef, double *zeta, double *inv2z, double *Px, double *Py,
+                                 double *Pz, double *PAx, double *PAy, double *PAz, double *cc)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const int g = pair_base + j;
+    const int sa = sha[g], sb = shb[g];
+    const double Ax = xyz[3 * sh_atom[sa]], Ay = xyz[3 * sh_atom[sa] + 1], Az = xyz[3 * sh_atom[sa] + 2];
+    const double Bx = xyz[3 * sh_atom[sb]], By = xyz[3 * sh_atom[sb] + 1], Bz = xyz[3 * sh_atom[sb] + 2];
+    const double AB2 = (Ax - Bx) * (Ax - Bx) + (Ay - By) * (Ay - By) + (Az - Bz) * (Az - Bz);
+    const int npa = sh_nprim[sa], npb = sh_nprim[sb];
+    const double c0 = 5.9149671727956128778;     // sqrt(2) * pi^(5/4)
+    for (int ia = 0; ia < npa; ++ia)
+        for (int ib = 0; ib < npb; ++ib) {
+            const double a = expo[sh_off[sa] + ia], b = expo[sh_off[sb] + ib];
+            const double z = a + b, iz = 1.0 / z;
+            const double px = (a * Ax + b * Bx) * iz, py = (a * Ay + b * By) * iz, pz = (a * Az + b * Bz) * iz;
+            const int idx = prim_base + (ia * npb + ib) * n + j;
+            zeta[idx] = z;  inv2z[idx] = 0.5 * iz;
+            Px[idx] = px;  Py[idx] = py;  Pz[idx] = pz;
+            PAx[idx] = px - Ax;  PAy[idx] = py - Ay;  PAz[idx] = pz - Az;
+            cc[idx] = c0 * coef[sh_off[sa] + ia] * coef[sh_off[sb] + ib] * exp(-a * b * iz * AB2) * iz;
+        }
+}
+
+// (a3) max|D| with non-finite detection.  out[0] = bit pattern of the max (non-negative doubles order like
+// their bit patterns), out[1] = 1 if any element is NaN/Inf.
+__global__ void dmax_kernel(const double *__restrict__ D, size_t n, unsigned long long *out)
+{
+    double m = 0.0;
+    int bad = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const double a = fabs(D[i]);
+        if (!(a <= DBL_MAX)) bad = 1;
+        m = fmax(m, a);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(out, (unsigned long long)__double_as_longlong(m));
+        if (bad) atomicOr(out + 1, 1ull);
+    }
+}
+
+// (a6) M <- M + M^T in place (M holds the one-sided accumulations of the digestion).
+__global__ void symmetrize_kernel(double *M, int N)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= N || j >= N || j > i) return;
+    const double a = M[(size_t)i * N + j], b = M[(size_t)j * N + i];
+    const double s = a + b;
+    M[(size_t)i * N + j] = s;
+    M[(size_t)j * N + i] = s;
+}
+
+// FP64 peak microbenchmark: 8 independent register-resident FMA chains per thread.
+__global__ void fp64_peak_kernel(double *out, int iters, double seed)
+{
+    double a0 = seed, a1 = seed + 1, a2 = seed + 2, a3 = seed + 3, a4 = seed + 4, a5 = seed + 5, a6 = seed + 6, a7 = seed + 7;
+    const double m = 0.999999, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 1234.5678) out[0] = s;      // never true; keeps the chains alive
+}
+
+}  // namespace adft
+
+using namespace adft;
+
+// ------------------------------------------------------------------ handles
+struct adft_basis {
+    int natoms = 0, nshells = 0, nbf = 0, nprim = 0;
+    std::vector<double> xyz, expo, coef;
+    std::vector<int32_t> atom, l, nprimv, off, bf_off;
+};
+
+struct Sublist {
+    int pc, la, lb, K, n, pair_base, prim_base;
+};
+
+struct adft_shellpairs {
+    const adft_basis *basis = nullptr;
+    int64_t npairs = 0, nprimpairs = 0;
+    std::vector<Sublist> subl;
+    std::vector<int> subl_of_class[NPAIRCLASS];
+    std::vector<double> hQ;            // sorted order
+    std::vector<double> Qmat;          // [nshells*nshells]
+    // device: basis
+    double *d_xyz = nullptr, *d_expo = nullptr, *d_coef = nullptr;
+    int32_t *d_atom = nullptr, *d_nprim = nullptr, *d_off = nullptr;
+    // device: pair table
+    double *d_Q = nullptr, *d_AB = nullptr /* 3*npairs */, *d_prim = nullptr /* 9*nprimpairs */;
+    int32_t *d_pint = nullptr /* 4*npairs: bfa,bfb,sha,shb */;
+    double *d_boys = nullptr;
+    PairTable tab{};
+    // per-build workspaces
+    Segment *d_segs = nullptr, *h_segs = nullptr;
+    size_t segs_cap = 0;
+    unsigned long long *d_counters = nullptr, *d_dmax = nullptr, *h_small = nullptr;
+    cudaEvent_t ev[2 * NQCLASS + 8] = {};
+    bool ev_ok = false;
+    // last build
+    adft_jk_stats_t stats{};
+    bool class_ran[NQCLASS] = {};
+    bool have_build = false;
+    cudaStream_t last_stream = nullptr;
+    // staging for adft_jk_build_host
+    double *d_stage = nullptr;
+    size_t stage_n = 0;
+    // sink for the output the caller skipped (J == NULL or K == NULL): round 1 has one kernel variant per class
+    double *d_sink = nullptr;
+};
+
+// ------------------------------------------------------------------ misc API
+extern "C" const char *adft_status_string(adft_status_t s)
+{
+    switch (s) {
+        case ADFT_OK: return "ok";
+        case ADFT_ERR_INVALID_ARG: return "invalid argument";
+        case ADFT_ERR_UNSUPPORTED_L: return "unsupported angular momentum";
+        case ADFT_ERR_ALLOC: return "allocation failed";
+        case ADFT_ERR_CUDA: return "CUDA error";
+        case ADFT_ERR_NOT_FINITE: return "density matrix is not finite";
+        case ADFT_ERR_INTERNAL: return "internal error";
+    }
+    return "unknown status";
+}
+extern "C" const char *adft_last_error(void) { return g_last_error.c_str(); }
+
+// ------------------------------------------------------------------ (a1) basis
+extern "C" adft_status_t adft_basis_create(int32_t natoms, const double *xyz, int32_t nshells, const adft_shell_t *shells,
+                                           const double *exponents, const double *coefficients, uint32_t flags,
+                                           adft_basis_t **out)
+{
+    if (!xyz || !shells || !exponents || !coefficients || !out || natoms <= 0 || nshells <= 0) {
+        set_error("adft_basis_create: NULL pointer or non-positive size");
+        return ADFT_ERR_INVALID_ARG;
+    }
+    if (flags & ~1u) { set_error("adft_basis_create: unknown flags"); return ADFT_ERR_INVALID_ARG; }
+    for (int i = 0; i < 3 * natoms; ++i)
+        if (!std::isfinite(xyz[i])) { set_error("adft_basis_create: non-finite coordinate"); return ADFT_ERR_INVALID_ARG; }
+    adft_basis *b = new (std::nothrow) adft_basis;
+    if (!b) return ADFT_ERR_ALLOC;
+    b->natoms = natoms; b->nshells = nshells;
+    b->xyz.assign(xyz, xyz + 3 * natoms);
+    b->bf_off.push_back(0);
+    for (int s = 0; s < nshells; ++s) {
+        const adft_shell_t &sh = shells[s];
+        if (sh.l < 0 || sh.l > 3) {
+            set_error("adft_basis_create: shell " + std::to_string(s) + " has l=" + std::to_string(sh.l) + " (supported 0..3)");
+            delete b; return ADFT_ERR_UNSUPPORTED_L;
+        }
+        if (sh.atom < 0 || sh.atom >= natoms || sh.nprim < 1 || sh.prim_offset < 0) {
+            set_error("adft_basis_create: shell " + std::to_string(s) + " has a bad atom index, nprim or offset");
+            delete b; return ADFT_ERR_INVALID_ARG;
+        }
+        b->atom.push_back(sh.atom); b->l.push_back(sh.l); b->nprimv.push_back(sh.nprim);
+        b->off.push_back((int32_t)b->expo.size());
+        for (int k = 0; k < sh.nprim; ++k) {
+            const double a = exponents[sh.prim_offset + k], c = coefficients[sh.prim_offset + k];
+            if (!(a > 0.0) || !std::isfinite(a) || !std::isfinite(c)) {
+                set_error("adft_basis_create: non-positive or non-finite exponent / coefficient in shell " + std::to_string(s));
+                delete b; return ADFT_ERR_INVALID_ARG;
+            }
+            b->expo.push_back(a); b->coef.push_back(c);
+        }
+        b->bf_off.push_back(b->bf_off.back() + ncart(sh.l));
+    }
+    b->nbf = b->bf_off.back();
+    b->nprim = (int)b->expo.size();
+    if (flags & ADFT_NORMALIZE_SHELLS) {
+        // DESIGN R-1: d_k = c_k N_k / sqrt(S); N_k norm of the (L,0,0) primitive, S contracted self-overlap of (L,0,0)
+        const double pi = 3.14159265358979323846;
+        for (int s = 0; s < nshells; ++s) {
+            const int L = b->l[s], o = b->off[s], n = b->nprimv[s];
+            double df = 1.0;
+            for (int k = 2 * L - 1; k > 1; k -= 2) df *= k;
+            for (int k = 0; k < n; ++k) {
+                const double a = b->expo[o + k];
+                b->coef[o + k] *= std::pow(2.0 * a / pi, 0.75) * std::pow(4.0 * a, 0.5 * L) / std::sqrt(df);
+            }
+            double S = 0.0;
+            for (int i = 0; i < n; ++i)
+                for (int j = 0; j < n; ++j) {
+                    const double p = b->expo[o + i] + b->expo[o + j];
+                    S += b->coef[o + i] * b->coef[o + j] * std::pow(pi / p, 1.5) * df / std::pow(2.0 * p, (double)L);
+                }
+            if (!(S > 0.0)) { set_error("adft_basis_create: shell with zero norm"); delete b; return ADFT_ERR_INVALID_ARG; }
+            const double r = 1.0 / std::sqrt(S);
+            for (int k = 0; k < n; ++k) b->coef[o + k] *= r;
+        }
+    }
+    *out = b;
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_basis_nbf(const adft_basis_t *b, int32_t *nbf)
+{
+    if (!b || !nbf) { set_error("adft_basis_nbf: NULL"); return ADFT_ERR_INVALID_ARG; }
+    *nbf = b->nbf;
+    return ADFT_OK;
+}
+extern "C" adft_status_t adft_basis_shell_offsets(const adft_basis_t *b, int32_t *bf_offset)
+{
+    if (!b || !bf_offset) { set_error("adft_basis_shell_offsets: NULL"); return ADFT_ERR_INVALID_ARG; }
+    std::copy(b->bf_off.begin(), b->bf_off.end(), bf_offset);
+    return ADFT_OK;
+}
+extern "C" adft_status_t adft_basis_coefficients(const adft_basis_t *b, double *c)
+{
+    if (!b || !c) { set_error("adft_basis_coefficients: NULL"); return ADFT_ERR_INVALID_ARG; }
+    std::copy(b->coef.begin(), b->coef.end(), c);
+    return ADFT_OK;
+}
+extern "C" void adft_basis_destroy(adft_basis_t *b) { delete b; }
+
+// ------------------------------------------------------------------ Boys table (library's own; long double series)
+static void fill_boys_table(std::vector<double> &tab)
+{
+    tab.assign((size_t)BOYS_NT * BOYS_NM, 0.0);
+    for (int k = 0; k < BOYS_NT; ++k) {
+        const long double T = (long double)k / 8.0L;
+        const long double eT = expl(-T);
+        for (int m = 0; m < BOYS_NM; ++m) {
+            // F_m(T) = exp(-T) sum_i (2T)^i / ((2m+1)(2m+3)...(2m+2i+1))
+            long double term = 1.0L / (2 * m + 1), sum = term;
+            for (int i = 1; i < 4000; ++i) {
+                term *= 2.0L * T / (2 * m + 2 * i + 1);
+                sum += term;
+                if (term < sum * 1e-21L) break;
+            }
+            tab[(size_t)k * BOYS_NM + m] = (double)(eT * sum);
+        }
+    }
+}
+
+// ------------------------------------------------------------------ (a2) shell pairs
+static void free_pairs(adft_shellpairs *p)
+{
+    if (!p) return;
+    cudaFree(p->d_xyz); cudaFree(p->d_expo); cudaFree(p->d_coef); cudaFree(p->d_atom); cudaFree(p->d_nprim);
+    cudaFree(p->d_off); cudaFree(p->d_Q); cudaFree(p->d_AB); cudaFree(p->d_prim); cudaFree(p->d_pint);
+    cudaFree(p->d_boys); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage); cudaFree(p->d_sink);
+    if (p->h_segs) cudaFreeHost(p->h_segs);
+    if (p->h_small) cudaFreeHost(p->h_small);
+    if (p->ev_ok) for (auto &e : p->ev) cudaEventDestroy(e);
+    delete p;
+}
+extern "C" void adft_shellpairs_destroy(adft_shellpairs_t *p) { free_pairs(p); }
+
+struct HostPair { int sa, sb; double Q; };
+
+static void set_table_pointers(adft_shellpairs *p)
+{
+    const size_t np = (size_t)p->npairs, npp = (size_t)p->nprimpairs;
+    PairTable &t = p->tab;
+    t.Q = p->d_Q;
+    t.ABx = p->d_AB; t.ABy = p->d_AB + np; t.ABz = p->d_AB + 2 * np;
+    t.bfa = p->d_pint; t.bfb = p->d_pint + np; t.sha = p->d_pint + 2 * np; t.shb = p->d_pint + 3 * np;
+    t.zeta = p->d_prim; t.inv2z = p->d_prim + npp; t.Px = p->d_prim + 2 * npp; t.Py = p->d_prim + 3 * npp;
+    t.Pz = p->d_prim + 4 * npp; t.PAx = p->d_prim + 5 * npp; t.PAy = p->d_prim + 6 * npp; t.PAz = p->d_prim + 7 * npp;
+    t.cc = p->d_prim + 8 * npp;
+}
+
+static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vector<HostPair> &hp, cudaStream_t st)
+{
+    const adft_basis *b = p->basis;
+    const size_t np = hp.size();
+    std::vector<double> AB(3 * np);
+    std::vector<int32_t> pint(4 * np);
+    for (size_t g = 0; g < np; ++g) {
+        const int sa = hp[g].sa, sb = hp[g].sb;
+        for (int i = 0; i < 3; ++i) AB[i * np + g] = b->xyz[3 * b->atom[sa] + i] - b->xyz[3 * b->atom[sb] + i];
+        pint[g] = b->bf_off[sa]; pint[np + g] = b->bf_off[sb]; pint[2 * np + g] = sa; pint[3 * np + g] = sb;
+    }
+    CUDA_TRY(cudaMemcpyAsync(p->d_AB, AB.data(), AB.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(p->d_pint, pint.data(), pint.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaStreamSynchronize(st));     // host vectors go out of scope
+    const size_t npp = (size_t)p->nprimpairs;
+    double *f = p->d_prim;
+    for (const Sublist &s : p->subl) {
+        if (s.n == 0) continue;
+        pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, p->tab.sha, p->tab.shb, p->d_atom,
+                                                             p->d_nprim, p->d_off, p->d_xyz, p->d_expo, p->d_coef, f, f + npp,
+                                                             f + 2 * npp, f + 3 * npp, f + 4 * npp, f + 5 * npp, f + 6 * npp,
+                                                             f + 7 * npp, f + 8 * npp);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda_stream, adft_shellpairs_t **out)
+{
+    if (!b || !out) { set_error("adft_shellpairs_build: NULL"); return ADFT_ERR_INVALID_ARG; }
+    ensure_registered();
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        set_error("adft_shellpairs_build: no CUDA device (there is no CPU fallback)");
+        return ADFT_ERR_CUDA;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    adft_shellpairs *p = new (std::nothrow) adft_shellpairs;
+    if (!p) return ADFT_ERR_ALLOC;
+    p->basis = b;
+    const int ns = b->nshells;
+
+    // bucket pairs (A >= B) by pair class and contraction depth; a = the higher-l shell
+    struct Key { int pc, K; bool operator<(const Key &o) const { return pc != o.pc ? pc < o.pc : K < o.K; } };
+    std::vector<std::pair<Key, HostPair>> all;
+    all.reserve((size_t)ns * (ns + 1) / 2);
+    for (int A = 0; A < ns; ++A)
+        for (int B = 0; B <= A; ++B) {
+            int sa = A, sb = B;
+            if (b->l[sa] < b->l[sb]) std::swap(sa, sb);
+            all.push_back({Key{pair_class(b->l[sa], b->l[sb]), b->nprimv[sa] * b->nprimv[sb]}, HostPair{sa, sb, 0.0}});
+        }
+    std::stable_sort(all.begin(), all.end(), [](const auto &x, const auto &y) { return x.first < y.first; });
+    std::vector<HostPair> hp(all.size());
+    p->npairs = (int64_t)all.size();
+    int64_t prim_total = 0;
+    for (size_t g = 0; g < all.size();) {
+        size_t e = g;
+        while (e < all.size() && !(all[g].first < all[e].first)) ++e;
+        Sublist s;
+        s.pc = all[g].first.pc; s.K = all[g].first.K; s.n = (int)(e - g);
+        s.la = b->l[all[g].second.sa]; s.lb = b->l[all[g].second.sb];
+        s.pair_base = (int)g; s.prim_base = (int)prim_total;
+        prim_total += (int64_t)s.K * s.n;
+        p->subl_of_class[s.pc].push_back((int)p->subl.size());
+        p->subl.push_back(s);
+        for (size_t q = g; q < e; ++q) hp[q] = all[q].second;
+        g = e;
+    }
+    if (prim_total > 0x7fffffffLL) { set_error("adft_shellpairs_build: too many primitive pairs"); free_pairs(p); return ADFT_ERR_ALLOC; }
+    p->nprimpairs = prim_total;
+    // every needed Schwarz class must exist
+    for (const Sublist &s : p->subl) {
+        const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
+        if (!ce.launch_schwarz) {
+            set_error("adft_shellpairs_build: no kernel for pair class (" + std::to_string(s.la) + "," + std::to_string(s.lb) + ")");
+            free_pairs(p); return ADFT_ERR_UNSUPPORTED_L;
+        }
+    }
+
+    const size_t np = (size_t)p->npairs, npp = (size_t)p->nprimpairs;
+#define ALLOC(ptr, bytes)                                                                                   \
+    if (cudaMalloc((void **)&(ptr), (bytes)) != cudaSuccess) {                                              \
+        set_error("adft_shellpairs_build: cudaMalloc of " + std::to_string((size_t)(bytes)) + " bytes failed"); \
+        cudaGetLastError(); free_pairs(p); return ADFT_ERR_ALLOC;                                           \
+    }
+    ALLOC(p->d_xyz, b->xyz.size() * sizeof(double));
+    ALLOC(p->d_expo, b->expo.size() * sizeof(double));
+    ALLOC(p->d_coef, b->coef.size() * sizeof(double));
+    ALLOC(p->d_atom, ns * sizeof(int32_t));
+    ALLOC(p->d_nprim, ns * sizeof(int32_t));
+    ALLOC(p->d_off, ns * sizeof(int32_t));
+    ALLOC(p->d_Q, np * sizeof(double));
+    ALLOC(p->d_AB, 3 * np * sizeof(double));
+    ALLOC(p->d_pint, 4 * np * sizeof(int32_t));
+    ALLOC(p->d_prim, 9 * npp * sizeof(double));
+    ALLOC(p->d_boys, (size_t)BOYS_NT * BOYS_NM * sizeof(double));
+    ALLOC(p->d_counters, 2 * NQCLASS * sizeof(unsigned long long));
+    ALLOC(p->d_dmax, 2 * sizeof(unsigned long long));
+#undef ALLOC
+    if (cudaMallocHost((void **)&p->h_small, 4 * NQCLASS * sizeof(unsigned long long)) != cudaSuccess) {
+        set_error("adft_shellpairs_build: cudaMallocHost failed"); free_pairs(p); return ADFT_ERR_ALLOC;
+    }
+    for (auto &e : p->ev)
+        if (cudaEventCreate(&e) != cudaSuccess) { set_error("cudaEventCreate failed"); free_pairs(p); return ADFT_ERR_CUDA; }
+    p->ev_ok = true;
+    set_table_pointers(p);
+
+    adft_status_t rc = ADFT_OK;
+    auto fail = [&](adft_status_t r) { free_pairs(p); return r; };
+#define TRY2(expr)                                                                         \
+    do {                                                                                   \
+        cudaError_t e__ = (expr);                                                          \
+        if (e__ != cudaSuccess) {                                                          \
+            set_error(std::string(#expr) + ": " + cudaGetErrorString(e__));                \
+            return fail(ADFT_ERR_CUDA);                                                    \
+        }                                                                                  \
+    } while (0)
+    TRY2(cudaMemcpyAsync(p->d_xyz, b->xyz.data(), b->xyz.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    TRY2(cudaMemcpyAsync(p->d_expo, b->expo.data(), b->expo.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    TRY2(cudaMemcpyAsync(p->d_coef, b->coef.data(), b->coef.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    TRY2(cudaMemcpyAsync(p->d_atom, b->atom.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    TRY2(cudaMemcpyAsync(p->d_nprim, b->nprimv.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    TRY2(cudaMemcpyAsync(p->d_off, b->off.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    std::vector<double> boys;
+    fill_boys_table(boys);
+    TRY2(cudaMemcpyAsync(p->d_boys, boys.data(), boys.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    TRY2(cudaStreamSynchronize(st));
+
+    // pass 1: records in bucket order, Schwarz bounds
+    rc = upload_pairs_and_prims(p, hp, st);
+    if (rc) return fail(rc);
+    for (const Sublist &s : p->subl) {
+        if (s.n == 0) continue;
+        class_table()[quartet_class(s.pc, s.pc)].launch_schwarz(p->tab, s.pair_base, s.prim_base, s.n, s.K, p->d_boys, p->d_Q, st);
+    }
+    TRY2(cudaGetLastError());
+    std::vector<double> Q(np);
+    TRY2(cudaMemcpyAsync(Q.data(), p->d_Q, np * sizeof(double), cudaMemcpyDeviceToHost, st));
+    TRY2(cudaStreamSynchronize(st));
+    for (size_t g = 0; g < np; ++g) {
+        if (!std::isfinite(Q[g])) { set_error("adft_shellpairs_build: non-finite Schwarz bound"); return fail(ADFT_ERR_INTERNAL); }
+        hp[g].Q = Q[g];
+    }
+    // pass 2: sort every sublist by Q descending (ties: by shell indices, for determinism) and rebuild the records
+    for (const Sublist &s : p->subl)
+        std::sort(hp.begin() + s.pair_base, hp.begin() + s.pair_base + s.n, [](const HostPair &x, const HostPair &y) {
+            if (x.Q != y.Q) return x.Q > y.Q;
+            if (x.sa != y.sa) return x.sa < y.sa;
+            return x.sb < y.sb;
+        });
+    p->hQ.resize(np);
+    p->Qmat.assign((size_t)ns * ns, 0.0);
+    for (size_t g = 0; g < np; ++g) {
+        p->hQ[g] = hp[g].Q;
+        p->Qmat[(size_t)hp[g].sa * ns + hp[g].sb] = p->Qmat[(size_t)hp[g].sb * ns + hp[g].sa] = hp[g].Q;
+    }
+    TRY2(cudaMemcpyAsync(p->d_Q, p->hQ.data(), np * sizeof(double), cudaMemcpyHostToDevice, st));
+    rc = upload_pairs_and_prims(p, hp, st);
+    if (rc) return fail(rc);
+    TRY2(cudaStreamSynchronize(st));
+#undef TRY2
+    *out = p;
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_shellpairs_schwarz(const adft_shellpairs_t *p, double *Q)
+{
+    if (!p || !Q) { set_error("adft_shellpairs_schwarz: NULL"); return ADFT_ERR_INVALID_ARG; }
+    std::copy(p->Qmat.begin(), p->Qmat.end(), Q);
+    return ADFT_OK;
+}
+extern "C" adft_status_t adft_shellpairs_counts(const adft_shellpairs_t *p, int64_t *npairs, int64_t *nprimpairs)
+{
+    if (!p) { set_error("adft_shellpairs_counts: NULL"); return ADFT_ERR_INVALID_ARG; }
+    if (npairs) *npairs = p->npairs;
+    if (nprimpairs) *nprimpairs = p->nprimpairs;
+    return ADFT_OK;
+}
+
+// ------------------------------------------------------------------ (a3) launch plan (host; Q lists are sorted descending)
+// number of leading elements q of a descending list with (qfix*q)*dmax >= tau   (monotone predicate, DESIGN R-7)
+static int prefix_len(const double *q, int n, double qfix, double dmax, double tau)
+{
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if ((qfix * q[mid]) * dmax >= tau) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax, double tau, std::vector<Segment> &segs)
+{
+    segs.clear();
+    for (int i1 : p->subl_of_class[X])
+        for (int i2 : p->subl_of_class[Y]) {
+            if (X == Y && i2 > i1) continue;
+            const Sublist &s1 = p->subl[i1], &s2 = p->subl[i2];
+            if (s1.n == 0 || s2.n == 0) continue;
+            const double *q1 = p->hQ.data() + s1.pair_base, *q2 = p->hQ.data() + s2.pair_base;
+            const int rows = prefix_len(q1, s1.n, q2[0], dmax, tau);
+            int cols = prefix_len(q2, s2.n, q1[0], dmax, tau);
+            const bool same = (i1 == i2);
+            if (same) cols = std::min(cols, rows);
+            if (rows == 0 || cols == 0) continue;
+            Segment sg{};
+            sg.bra_pair_base = s1.pair_base; sg.bra_prim_base = s1.prim_base; sg.bra_n = s1.n; sg.bra_K = s1.K;
+            sg.ket_pair_base = s2.pair_base; sg.ket_prim_base = s2.prim_base; sg.ket_n = s2.n; sg.ket_K = s2.K;
+            sg.rows = rows; sg.tiles_per_row = (cols + 31) / 32; sg.same = same ? 1 : 0;
+            segs.push_back(sg);
+        }
+    // heaviest tiles first (per-tile cost ~ K1*K2), so the tail of the launch is made of cheap tiles
+    std::stable_sort(segs.begin(), segs.end(), [](const Segment &a, const Segment &b) {
+        return (long long)a.bra_K * a.ket_K > (long long)b.bra_K * b.ket_K;
+    });
+    long long w = 0;
+    for (Segment &s : segs) { s.warp_begin = w; w += (long long)s.rows * s.tiles_per_row; }
+    return w;
+}
+
+// ------------------------------------------------------------------ the J/K build
+extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, double *J, double *K, double tau,
+                                       void *cuda_stream)
+{
+    if (!p || !D || (!J && !K)) { set_error("adft_jk_build: NULL handle or D, or both J and K NULL"); return ADFT_ERR_INVALID_ARG; }
+    if (!(tau >= 0.0) || !std::isfinite(tau)) { set_error("adft_jk_build: schwarz_threshold must be finite and >= 0"); return ADFT_ERR_INVALID_ARG; }
+    if (D == J || D == K) { set_error("adft_jk_build: D must not alias J or K"); return ADFT_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int N = p->basis->nbf;
+    const size_t n2 = (size_t)N * N;
+    int launches = 0;
+    // every class that can occur must have a kernel
+    for (int X = 0; X < NPAIRCLASS; ++X)
+        for (int Y = 0; Y <= X; ++Y)
+            if (!p->subl_of_class[X].empty() && !p->subl_of_class[Y].empty() && !class_table()[quartet_class(X, Y)].launch_jk) {
+                set_error("adft_jk_build: no kernel compiled for quartet class " + std::to_string(quartet_class(X, Y)));
+                return ADFT_ERR_UNSUPPORTED_L;
+            }
+    if ((!J || !K) && !p->d_sink) CUDA_TRY(cudaMalloc((void **)&p->d_sink, n2 * sizeof(double)));
+    double *Jw = J ? J : p->d_sink, *Kw = K ? K : p->d_sink;
+    cudaEvent_t *ev = p->ev;
+    cudaEvent_t ev_begin = ev[2 * NQCLASS], ev_dmax = ev[2 * NQCLASS + 1], ev_plan = ev[2 * NQCLASS + 2],
+                ev_eri = ev[2 * NQCLASS + 3], ev_end = ev[2 * NQCLASS + 4];
+    CUDA_TRY(cudaEventRecord(ev_begin, st));
+    // (a3) Dmax
+    CUDA_TRY(cudaMemsetAsync(p->d_dmax, 0, 2 * sizeof(unsigned long long), st));
+    dmax_kernel<<<592, 256, 0, st>>>(D, n2, p->d_dmax); ++launches;
+    CUDA_TRY(cudaMemcpyAsync(p->h_small, p->d_dmax, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaEventRecord(ev_dmax, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (p->h_small[1]) { set_error("adft_jk_build: D contains NaN or Inf"); return ADFT_ERR_NOT_FINITE; }
+    double dmax;
+    std::memcpy(&dmax, &p->h_small[0], sizeof(double));
+
+    // plan: segments of every class
+    std::vector<std::vector<Segment>> plan(NQCLASS);
+    long long warps[NQCLASS] = {};
+    size_t nseg_total = 0;
+    for (int X = 0; X < NPAIRCLASS; ++X)
+        for (int Y = 0; Y <= X; ++Y) {
+            const int qc = quartet_class(X, Y);
+            warps[qc] = plan_class(p, X, Y, dmax, tau, plan[qc]);
+            nseg_total += plan[qc].size();
+        }
+    if (nseg_total > p->segs_cap) {
+        cudaFree(p->d_segs); if (p->h_segs) cudaFreeHost(p->h_segs);
+        p->d_segs = nullptr; p->h_segs = nullptr; p->segs_cap = 0;
+        const size_t cap = nseg_total + nseg_total / 4 + 64;
+        CUDA_TRY(cudaMalloc((void **)&p->d_segs, cap * sizeof(Segment)));
+        CUDA_TRY(cudaMallocHost((void **)&p->h_segs, cap * sizeof(Segment)));
+        p->segs_cap = cap;
+    }
+    size_t seg_off[NQCLASS] = {};
+    {
+        size_t o = 0;
+        for (int qc = 0; qc < NQCLASS; ++qc) {
+            seg_off[qc] = o;
+            std::copy(plan[qc].begin(), plan[qc].end(), p->h_segs + o);
+            o += plan[qc].size();
+        }
+        if (o) CUDA_TRY(cudaMemcpyAsync(p->d_segs, p->h_segs, o * sizeof(Segment), cudaMemcpyHostToDevice, st));
+    }
+    CUDA_TRY(cudaMemsetAsync(p->d_counters, 0, 2 * NQCLASS * sizeof(unsigned long long), st));
+    if (J) CUDA_TRY(cudaMemsetAsync(J, 0, n2 * sizeof(double), st));
+    if (K) CUDA_TRY(cudaMemsetAsync(K, 0, n2 * sizeof(double), st));
+    CUDA_TRY(cudaEventRecord(ev_plan, st));
+
+    // (a4)+(a5) one launch per class, heavy classes first
+    int order[NQCLASS];
+    std::iota(order, order + NQCLASS, 0);
+    std::stable_sort(order, order + NQCLASS, [&](int a, int b) { return a > b; });
+    for (int qi = 0; qi < NQCLASS; ++qi) {
+        const int qc = order[qi];
+        p->class_ran[qc] = false;
+        if (warps[qc] == 0) continue;
+        JKParams prm{};
+        prm.t = p->tab; prm.segs = p->d_segs + seg_off[qc]; prm.nsegs = (int)plan[qc].size(); prm.total_warps = warps[qc];
+        prm.D = D; prm.J = Jw; prm.K = Kw; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boys;
+        prm.counters = p->d_counters + 2 * qc;
+        CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
+        class_table()[qc].launch_jk(prm, st, J != nullptr, K != nullptr); ++launches;
+        CUDA_TRY(cudaEventRecord(ev[2 * qc + 1], st));
+        p->class_ran[qc] = true;
+    }
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaEventRecord(ev_eri, st));
+    // (a6) finalise
+    dim3 blk(32, 8), grd((N + 31) / 32, (N + 7) / 8);
+    if (J) { symmetrize_kernel<<<grd, blk, 0, st>>>(J, N); ++launches; }
+    if (K) { symmetrize_kernel<<<grd, blk, 0, st>>>(K, N); ++launches; }
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaEventRecord(ev_end, st));
+    p->stats = adft_jk_stats_t{};
+    p->stats.dmax = dmax;
+    p->stats.quartets_unique = p->npairs * (p->npairs + 1) / 2;
+    p->stats.kernel_launches = launches;
+    p->have_build = true;
+    p->last_stream = st;
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_jk_stats(adft_shellpairs_t *p, adft_jk_stats_t *out)
+{
+    if (!p || !out) { set_error("adft_jk_stats: NULL"); return ADFT_ERR_INVALID_ARG; }
+    if (!p->have_build) { set_error("adft_jk_stats: no build yet"); return ADFT_ERR_INVALID_ARG; }
+    cudaStream_t st = p->last_stream;
+    CUDA_TRY(cudaMemcpyAsync(p->h_small, p->d_counters, 2 * NQCLASS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    adft_jk_stats_t &s = p->stats;
+    cudaEvent_t *ev = p->ev;
+    s.quartets_kept = 0; s.prim_quartets = 0; s.model_flops = 0.0;
+    for (int qc = 0; qc < NQCLASS; ++qc) {
+        s.class_quartets[qc] = (int64_t)p->h_small[2 * qc];
+        const int64_t prim = (int64_t)p->h_small[2 * qc + 1];
+        s.quartets_kept += s.class_quartets[qc];
+        s.prim_quartets += prim;
+        const ClassEntry &ce = class_table()[qc];
+        const int L = ce.la + ce.lb + ce.lc + ce.ld;
+        // model flops: per primitive quartet 60+4L (geometry, prefactor, Boys) + generated VRR instructions
+        // counted as 2 flops each; per contracted quartet 2*HRR + 12 per integral (6 FMAs of the digestion)
+        s.model_flops += (double)prim * (60.0 + 4.0 * L + 2.0 * ce.vrr_ops)
+                       + (double)s.class_quartets[qc] * (2.0 * ce.hrr_ops + 12.0 * ce.nint);
+        float ms = 0.f;
+        s.class_ms[qc] = 0.0;
+        if (p->class_ran[qc] && cudaEventElapsedTime(&ms, ev[2 * qc], ev[2 * qc + 1]) == cudaSuccess) s.class_ms[qc] = ms;
+    }
+    float ms = 0.f;
+    const int B = 2 * NQCLASS;
+    if (cudaEventElapsedTime(&ms, ev[B], ev[B + 1]) == cudaSuccess) s.ms_dmax = ms;
+    if (cudaEventElapsedTime(&ms, ev[B + 1], ev[B + 2]) == cudaSuccess) s.ms_plan = ms;
+    if (cudaEventElapsedTime(&ms, ev[B + 2], ev[B + 3]) == cudaSuccess) s.ms_eri = ms;
+    if (cudaEventElapsedTime(&ms, ev[B + 3], ev[B + 4]) == cudaSuccess) s.ms_finalize = ms;
+    if (cudaEventElapsedTime(&ms, ev[B], ev[B + 4]) == cudaSuccess) s.ms_total = ms;
+    cudaGetLastError();
+    *out = s;
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_jk_build_host(adft_shellpairs_t *p, const double *Dh, double *Jh, double *Kh, double tau,
+                                            void *cuda_stream)
+{
+    if (!p || !Dh || (!Jh && !Kh)) { set_error("adft_jk_build_host: NULL handle or D, or both J and K NULL"); return ADFT_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n2 = (size_t)p->basis->nbf * p->basis->nbf;
+    if (p->stage_n < 3 * n2) {
+        cudaFree(p->d_stage); p->d_stage = nullptr; p->stage_n = 0;
+        CUDA_TRY(cudaMalloc((void **)&p->d_stage, 3 * n2 * sizeof(double)));
+        p->stage_n = 3 * n2;
+    }
+    double *dD = p->d_stage, *dJ = Jh ? p->d_stage + n2 : nullptr, *dK = Kh ? p->d_stage + 2 * n2 : nullptr;
+    CUDA_TRY(cudaMemcpyAsync(dD, Dh, n2 * sizeof(double), cudaMemcpyHostToDevice, st));
+    adft_status_t rc = adft_jk_build(p, dD, dJ, dK, tau, cuda_stream);
+    if (rc) return rc;
+    if (Jh) CUDA_TRY(cudaMemcpyAsync(Jh, dJ, n2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (Kh) CUDA_TRY(cudaMemcpyAsync(Kh, dK, n2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_fp64_peak_tflops(void *cuda_stream, double *tflops)
+{
+    if (!tflops) { set_error("adft_fp64_peak_tflops: NULL"); return ADFT_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double *d = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&d, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0)); CUDA_TRY(cudaEventCreate(&e1));
+    const int iters = 1 << 16, blocks = sms * 8, threads = 256;
+    fp64_peak_kernel<<<blocks, threads, 0, st>>>(d, 1 << 10, 1.0);       // warm-up
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, st);
+        fp64_peak_kernel<<<blocks, threads, 0, st>>>(d, iters, 1.0 + rep);
+        cudaEventRecord(e1, st);
+        CUDA_TRY(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        const double fl = 2.0 * 8.0 * (double)iters * blocks * threads;
+        best = std::max(best, fl / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    *tflops = best;
+    return ADFT_OK;
+}
