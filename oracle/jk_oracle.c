@@ -1,6 +1,7 @@
 /* ORACLE -- TEST INFRASTRUCTURE ONLY.
  *
- * Plain, slow, fp64 CPU implementation of what the J/K hot path computes.  Only tests/,
+ * Plain, slow CPU implementation of what the J/K hot path computes: fp64 inputs and outputs, integral core
+ * and accumulators in long double (>= fp64; R-12, R-19) so that the whole error budget is the GPU's.  Only tests/,
  * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call it.
  * It shares no code, tables or constants with the CUDA library (paper_2406_11185_b200/csrc).
  *
@@ -162,6 +163,17 @@ int orc_eri_block_ld(BASIS_ARGS, int sA, int sB, int sC, int sD, long double *ou
     return 0;
 }
 
+/* The oracle proper (Schwarz table, J/K, blocks) evaluates the integral core in long double and keeps the
+ * integrals in long double through the J/K accumulation; only the outputs are fp64 (reading R-19).  Reason: in the oracle's fixed input shell order the plain
+ * fp64 HRR, (a,b+1_i| = (a+1_i,b| + (A_i-B_i)(ab|, cancels badly when angular momentum is shifted from a distant
+ * diffuse shell onto a tight high-l shell (measured: cfg 1 shells (35,23): Q_fp64 3.003293e-4, Q_long-double
+ * 3.003267e-4).  The fp64 instantiation is kept for pin P13 and for orc_eri_block. */
+#define CORE_REAL long double
+#define core_scratch_t scratch_t_ld
+#define core_scratch_alloc scratch_alloc_ld
+#define core_scratch_free scratch_free_ld
+#define core_shell_quartet shell_quartet_ld
+
 /* ---- exported: Schwarz bounds Q[nshells*nshells] (SURVEY R-10) ---- */
 int orc_schwarz(BASIS_ARGS, double *Q)
 {
@@ -170,9 +182,9 @@ int orc_schwarz(BASIS_ARGS, double *Q)
     int err = 0;
 #pragma omp parallel
     {
-        scratch_t_d s;
-        double *blk = (double *)malloc(sizeof(double) * 10000);
-        if (scratch_alloc_d(&s) || !blk) {
+        core_scratch_t s;
+        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * 10000);
+        if (core_scratch_alloc(&s) || !blk) {
 #pragma omp atomic write
             err = -3;
         } else {
@@ -180,17 +192,17 @@ int orc_schwarz(BASIS_ARGS, double *Q)
             for (int A = 0; A < nshells; ++A)
                 for (int B = 0; B <= A; ++B) {
                     int nA = NCART(l[A]), nB = NCART(l[B]);
-                    shell_quartet_d(&b, A, B, A, B, &s, blk);
+                    core_shell_quartet(&b, A, B, A, B, &s, blk);
                     double mx = 0.0;
                     for (int i = 0; i < nA; ++i)
                         for (int j = 0; j < nB; ++j) {
-                            double vdiag = fabs(blk[((i * nB + j) * nA + i) * nB + j]);
+                            double vdiag = fabs((double)blk[((i * nB + j) * nA + i) * nB + j]);
                             if (vdiag > mx) mx = vdiag;
                         }
                     Q[(size_t)A * nshells + B] = Q[(size_t)B * nshells + A] = sqrt(mx);
                 }
         }
-        scratch_free_d(&s); free(blk);
+        core_scratch_free(&s); free(blk);
     }
     return err;
 }
@@ -244,13 +256,13 @@ int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J
     int err = 0;
 #pragma omp parallel
     {
-        scratch_t_d s;
-        double *blk = (double *)malloc(sizeof(double) * 10000);
+        core_scratch_t s;
+        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * 10000);
         long double *Jp = (long double *)calloc((size_t)N * N, sizeof(long double));
         long double *Kp = (long double *)calloc((size_t)N * N, sizeof(long double));
         int64_t my_all = 0, my_kept = 0, my_prim = 0, mycc[55];
         memset(mycc, 0, sizeof mycc);
-        if (scratch_alloc_d(&s) || !blk || !Jp || !Kp) {
+        if (core_scratch_alloc(&s) || !blk || !Jp || !Kp) {
 #pragma omp atomic write
             err = -3;
         } else {
@@ -272,7 +284,7 @@ int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J
                         ++my_kept;
                         my_prim += (int64_t)nprim[A] * nprim[B] * nprim[C] * nprim[Dd];
                         ++mycc[qclass(l[A], l[B], l[C], l[Dd])];
-                        shell_quartet_d(&b, A, B, C, Dd, &s, blk);
+                        core_shell_quartet(&b, A, B, C, Dd, &s, blk);
                         double f = (A == B ? 0.5 : 1.0) * (C == Dd ? 0.5 : 1.0) * (pab == pcd ? 0.5 : 1.0);
                         int nA = NCART(l[A]), nB = NCART(l[B]), nC = NCART(l[C]), nD = NCART(l[Dd]);
                         for (int ia = 0; ia < nA; ++ia)
@@ -303,7 +315,7 @@ int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J
                 for (int i = 0; i < 55; ++i) cc[i] += mycc[i];
             }
         }
-        scratch_free_d(&s); free(blk); free(Jp); free(Kp);
+        core_scratch_free(&s); free(blk); free(Jp); free(Kp);
     }
     for (size_t i = 0; i < (size_t)N * N; ++i) { J[i] = (double)Jt[i]; K[i] = (double)Kt[i]; }
     if (counts) { counts[0] = n_all; counts[1] = n_kept; counts[2] = n_prim; }
@@ -349,12 +361,12 @@ int orc_jk_brute(BASIS_ARGS, const double *D, double *J, double *K)
     const int N = bo[nshells];
     long double *Jt = (long double *)calloc((size_t)N * N, sizeof(long double));
     long double *Kt = (long double *)calloc((size_t)N * N, sizeof(long double));
-    scratch_t_d s;
-    double *blk = (double *)malloc(sizeof(double) * 10000);
-    if (scratch_alloc_d(&s)) return -3;
+    core_scratch_t s;
+    CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * 10000);
+    if (core_scratch_alloc(&s)) return -3;
     for (int A = 0; A < nshells; ++A) for (int B = 0; B < nshells; ++B)
     for (int C = 0; C < nshells; ++C) for (int Dd = 0; Dd < nshells; ++Dd) {
-        shell_quartet_d(&b, A, B, C, Dd, &s, blk);
+        core_shell_quartet(&b, A, B, C, Dd, &s, blk);
         int nA = NCART(l[A]), nB = NCART(l[B]), nC = NCART(l[C]), nD = NCART(l[Dd]);
         for (int ia = 0; ia < nA; ++ia) for (int ib = 0; ib < nB; ++ib)
         for (int ic = 0; ic < nC; ++ic) for (int id = 0; id < nD; ++id) {
@@ -365,7 +377,7 @@ int orc_jk_brute(BASIS_ARGS, const double *D, double *J, double *K)
         }
     }
     for (size_t i = 0; i < (size_t)N * N; ++i) { J[i] = (double)Jt[i]; K[i] = (double)Kt[i]; }
-    scratch_free_d(&s); free(blk); free(Jt); free(Kt); free(bo);
+    core_scratch_free(&s); free(blk); free(Jt); free(Kt); free(bo);
     return 0;
 }
 
@@ -387,11 +399,11 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
     int err = 0;
 #pragma omp parallel
     {
-        scratch_t_d s;
-        double *blk = (double *)malloc(sizeof(double) * 10000);
+        core_scratch_t s;
+        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * 10000);
         long double Jp[100], Kp[100];
         for (int i = 0; i < 100; ++i) Jp[i] = Kp[i] = 0;
-        if (scratch_alloc_d(&s) || !blk) {
+        if (core_scratch_alloc(&s) || !blk) {
 #pragma omp atomic write
             err = -3;
         } else {
@@ -400,7 +412,7 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
                 for (int Dd = 0; Dd < nshells; ++Dd) {
                     int nC = NCART(l[C]), nD = NCART(l[Dd]);
                     if (Jblk && (Q[(size_t)sA * nshells + sB] * Q[(size_t)C * nshells + Dd]) * Dmax >= tau) {
-                        shell_quartet_d(&b, sA, sB, C, Dd, &s, blk);
+                        core_shell_quartet(&b, sA, sB, C, Dd, &s, blk);
                         for (int ia = 0; ia < nA; ++ia) for (int ib = 0; ib < nB; ++ib)
                         for (int ic = 0; ic < nC; ++ic) for (int id = 0; id < nD; ++id)
                             Jp[ia * nB + ib] += (long double)D[(size_t)(bo[C] + ic) * N + bo[Dd] + id]
@@ -408,7 +420,7 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
                     }
                     if (Kblk && (Q[(size_t)sA * nshells + C] * Q[(size_t)sB * nshells + Dd]) * Dmax >= tau) {
                         /* (A C | B D): mu in A, nu in C, lambda in B, sigma in D */
-                        shell_quartet_d(&b, sA, C, sB, Dd, &s, blk);
+                        core_shell_quartet(&b, sA, C, sB, Dd, &s, blk);
                         for (int ia = 0; ia < nA; ++ia) for (int ic = 0; ic < nC; ++ic)
                         for (int ib = 0; ib < nB; ++ib) for (int id = 0; id < nD; ++id)
                             Kp[ia * nB + ib] += (long double)D[(size_t)(bo[C] + ic) * N + bo[Dd] + id]
@@ -418,7 +430,7 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
 #pragma omp critical
             for (int i = 0; i < nA * nB; ++i) { Jt[i] += Jp[i]; Kt[i] += Kp[i]; }
         }
-        scratch_free_d(&s); free(blk);
+        core_scratch_free(&s); free(blk);
     }
     for (int i = 0; i < nA * nB; ++i) { if (Jblk) Jblk[i] = (double)Jt[i]; if (Kblk) Kblk[i] = (double)Kt[i]; }
     free(bo);

@@ -320,3 +320,22 @@ def test_p13_long_double_agreement(orc):
     b3 = orc.basis_from_workload(w3)
     d = orc.eri_block(b3, 0, 1, 2, 3); ld = orc.eri_block(b3, 0, 1, 2, 3, long_double=True)
     assert np.abs(ld - d).max() <= 1e-12 * np.abs(d).max()
+
+
+def test_p13_documented_hrr_cancellation_case(orc):
+    """DESIGN.md R-19: cfg 1 shells (35, 23) -- a diffuse p shell 8.5 bohr from a tight d shell.  The plain fp64 core
+    loses digits there (HRR shifts angular momentum onto the tight shell); the long-double core, which the oracle
+    proper uses, does not depend on the order the two shells are given in."""
+    w = W.make(1)
+    bs = orc.basis_from_workload(w)
+    A, B = 35, 23
+    ld1 = orc.eri_block(bs, A, B, A, B, long_double=True)
+    ld2 = orc.eri_block(bs, B, A, B, A, long_double=True).transpose(1, 0, 3, 2)
+    scale = float(np.abs(ld1).max())
+    assert float(np.abs(ld1 - ld2).max()) <= 1e-14                  # order-independent to 1e-14 absolute in long double
+    assert scale < 1e-6
+    d1 = orc.eri_block(bs, A, B, A, B)
+    assert float(np.abs(d1 - ld1.astype(np.float64)).max()) <= 1e-10  # fp64 core: absolute error stays tiny ...
+    Q = orc.schwarz(bs)
+    diag = max(float(abs(ld1[i, j, i, j])) for i in range(ld1.shape[0]) for j in range(ld1.shape[1]))
+    assert Q[A, B] == pytest.approx(np.sqrt(diag), rel=1e-13)         # ... and the Schwarz table uses the ld core
