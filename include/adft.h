@@ -69,6 +69,7 @@ typedef struct {
     int64_t class_quartets[ADFT_MAX_CLASSES]; /* kept per class; class = X(X+1)/2+Y, X >= Y pair classes,
                                                  pair class = hi(hi+1)/2+lo of the two angular momenta */
     double  class_ms[ADFT_MAX_CLASSES];       /* device time of each class kernel (CUDA events) */
+    double  class_model_flops[ADFT_MAX_CLASSES]; /* model FP64 flops of each class launch */
     double  model_flops;          /* FP64 flops of the generated recurrences for the kept work */
     double  dmax;                 /* max|D| used by the screen */
     double  ms_dmax, ms_plan, ms_eri, ms_finalize, ms_total; /* device ms; ms_total = whole call */

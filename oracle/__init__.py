@@ -166,14 +166,17 @@ def jk_brute(bs: Basis, D):
     return J, K
 
 
-def jk_block(bs: Basis, D, tau, Q, Dmax, A, B, want_j=True, want_k=True):
+def jk_block(bs: Basis, D, tau, Q, Dmax, A, B, want_j=True, want_k=True, with_work=False):
     D = np.ascontiguousarray(D, np.float64); Q = np.ascontiguousarray(Q, np.float64)
     Jb = np.zeros((bs.ncart[A], bs.ncart[B])); Kb = np.zeros((bs.ncart[A], bs.ncart[B]))
+    work = np.zeros(2, dtype=np.int64)
     rc = lib().orc_jk_block(*bs.args(), _p(D, C.c_double), C.c_double(tau), _p(Q, C.c_double), C.c_double(Dmax),
                             C.c_int(A), C.c_int(B), _p(Jb, C.c_double) if want_j else None,
-                            _p(Kb, C.c_double) if want_k else None)
+                            _p(Kb, C.c_double) if want_k else None, _p(work, C.c_int64))
     if rc:
         raise ValueError(f"orc_jk_block rc={rc}")
+    if with_work:
+        return Jb, Kb, (int(work[0]), int(work[1]))
     return Jb, Kb
 
 

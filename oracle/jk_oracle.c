@@ -386,8 +386,9 @@ int orc_jk_brute(BASIS_ARGS, const double *D, double *J, double *K)
  * Kblk[nA*nB]:  K_ml = sum_{C,D} [ (Q_AC*Q_BD)*Dmax >= tau ] sum_{n in C, s in D} D_ns (m n|l s), m in A, l in B
  * (the screen is symmetric under the 8 permutations, so this equals the block of orc_jk's result). */
 int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, double Dmax,
-                 int sA, int sB, double *Jblk, double *Kblk)
+                 int sA, int sB, double *Jblk, double *Kblk, int64_t *work /* [2]: shell quartets, primitive quartets evaluated; may be NULL */)
 {
+    int64_t w_q = 0, w_p = 0;
     basis_t b = mk_basis(BASIS_PASS);
     if (check_basis(&b)) return check_basis(&b);
     int *bo = (int *)malloc(sizeof(int) * (nshells + 1));
@@ -413,6 +414,10 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
                     int nC = NCART(l[C]), nD = NCART(l[Dd]);
                     if (Jblk && (Q[(size_t)sA * nshells + sB] * Q[(size_t)C * nshells + Dd]) * Dmax >= tau) {
                         core_shell_quartet(&b, sA, sB, C, Dd, &s, blk);
+#pragma omp atomic
+                        w_q += 1;
+#pragma omp atomic
+                        w_p += (int64_t)nprim[sA] * nprim[sB] * nprim[C] * nprim[Dd];
                         for (int ia = 0; ia < nA; ++ia) for (int ib = 0; ib < nB; ++ib)
                         for (int ic = 0; ic < nC; ++ic) for (int id = 0; id < nD; ++id)
                             Jp[ia * nB + ib] += (long double)D[(size_t)(bo[C] + ic) * N + bo[Dd] + id]
@@ -421,6 +426,10 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
                     if (Kblk && (Q[(size_t)sA * nshells + C] * Q[(size_t)sB * nshells + Dd]) * Dmax >= tau) {
                         /* (A C | B D): mu in A, nu in C, lambda in B, sigma in D */
                         core_shell_quartet(&b, sA, C, sB, Dd, &s, blk);
+#pragma omp atomic
+                        w_q += 1;
+#pragma omp atomic
+                        w_p += (int64_t)nprim[sA] * nprim[C] * nprim[sB] * nprim[Dd];
                         for (int ia = 0; ia < nA; ++ia) for (int ic = 0; ic < nC; ++ic)
                         for (int ib = 0; ib < nB; ++ib) for (int id = 0; id < nD; ++id)
                             Kp[ia * nB + ib] += (long double)D[(size_t)(bo[C] + ic) * N + bo[Dd] + id]
@@ -433,6 +442,7 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
         core_scratch_free(&s); free(blk);
     }
     for (int i = 0; i < nA * nB; ++i) { if (Jblk) Jblk[i] = (double)Jt[i]; if (Kblk) Kblk[i] = (double)Kt[i]; }
+    if (work) { work[0] = w_q; work[1] = w_p; }
     free(bo);
     return err;
 }

@@ -32,6 +32,7 @@ class AdftError(RuntimeError):
 class JKStats(C.Structure):
     _fields_ = [("quartets_unique", C.c_int64), ("quartets_kept", C.c_int64), ("prim_quartets", C.c_int64),
                 ("class_quartets", C.c_int64 * ADFT_MAX_CLASSES), ("class_ms", C.c_double * ADFT_MAX_CLASSES),
+                ("class_model_flops", C.c_double * ADFT_MAX_CLASSES),
                 ("model_flops", C.c_double), ("dmax", C.c_double),
                 ("ms_dmax", C.c_double), ("ms_plan", C.c_double), ("ms_eri", C.c_double),
                 ("ms_finalize", C.c_double), ("ms_total", C.c_double),
