@@ -620,7 +620,7 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         JKParams prm{};
         prm.t = p->tab; prm.segs = p->d_segs + seg_off[qc]; prm.nsegs = (int)plan[qc].size(); prm.total_warps = warps[qc];
         prm.D = D; prm.J = Jw; prm.K = Kw; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boys;
-        prm.counters = p->d_counters + 2 * qc;
+        prm.counters = p->d_counters + 2 * qc; prm.zero = 0;
         CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
         class_table()[qc].launch_jk(prm, st, J != nullptr, K != nullptr); ++launches;
         CUDA_TRY(cudaEventRecord(ev[2 * qc + 1], st));

@@ -62,6 +62,12 @@ def choose_dir(vec, how):
     raise ValueError(how)
 
 
+def all_targets(la, lb, lc, ld):
+    """(a, c) of every contracted [e0|f0] the HRR needs, in global accumulator order."""
+    return [(a, c) for dega in range(la, la + lb + 1) for a in comps(dega)
+            for degc in range(lc, lc + ld + 1) for c in comps(degc)]
+
+
 class VrrDag:
     """Vertical recurrences for one primitive quartet.
 
@@ -70,18 +76,15 @@ class VrrDag:
                              + a_i/(2(zeta+eta)) [a-1_i|c]^(m+1)
     """
 
-    def __init__(self, la, lb, lc, ld, how="first"):
+    def __init__(self, la, lb, lc, ld, how="first", targets=None):
         self.la, self.lb, self.lc, self.ld = la, lb, lc, ld
         self.lab, self.lcd = la + lb, lc + ld
         self.L = self.lab + self.lcd
         self.how = how
         self.nodes = OrderedDict()       # key -> spec ; insertion order is a valid topological order
-        self.targets = []                # (a, c) in acc order
-        for dega in range(la, self.lab + 1):
-            for a in comps(dega):
-                for degc in range(lc, self.lcd + 1):
-                    for c in comps(degc):
-                        self.targets.append((a, c))
+        if targets is None:              # all [e0|f0], in acc order
+            targets = all_targets(la, lb, lc, ld)
+        self.targets = list(targets)     # (a, c); position in this list = accumulator index of the pass
         for (a, c) in self.targets:
             self._need(("V", a, c, 0))
         self.ids = {k: i for i, k in enumerate(self.nodes)}
@@ -204,7 +207,7 @@ class VrrDag:
                     e = f"fma(kx{nx}, {name(tx)}, {e})"
                 out.append(f"    const double {v} = {e};")
             if key in tgt_index:
-                out.append(f"    acc[{tgt_index[key]}] += {v};")
+                out.append(f"    acc.template add<{tgt_index[key]}>({v});")
 
 
 class HrrDag:
@@ -280,7 +283,7 @@ class HrrDag:
         def name(k):
             s = self.nodes[k]
             if s[0] == "acc":
-                return f"acc[{s[1]}]"
+                return f"acc.template get<{s[1]}>()"
             if s[0] == "alias":
                 return name(s[1])
             return f"h{self.ids[k]}"
@@ -309,16 +312,40 @@ def class_tag(la, lb, lc, ld):
     return f"{la}{lb}{lc}{ld}"
 
 
-def best_vrr(la, lb, lc, ld):
+def best_vrr(la, lb, lc, ld, targets=None):
     best = None
     for how in ("first", "last", "max", "min"):
-        d = VrrDag(la, lb, lc, ld, how)
+        d = VrrDag(la, lb, lc, ld, how, targets)
         if best is None or d.fp64_ops() < best.fp64_ops():
             best = d
     return best
 
 
-def generate_class(la, lb, lc, ld):
+PREAMBLE_OPS = 70     # geometry, prefactor and Boys of one primitive quartet, repeated in every pass
+
+
+def plan_passes(la, lb, lc, ld, cmax):
+    """Multi-pass pruned VRR: partition the [e0|f0] targets into chunks of at most ~cmax accumulators (a chunk =
+    a group of bra degrees x a run of ket components) and re-walk, per chunk, only the part of the DAG it needs.
+    Returns the list of VrrDag (one per pass) with the smallest total FP64 op count among a few partitions."""
+    edegs = list(range(la, la + lb + 1))
+    clist = [c for degc in range(lc, lc + ld + 1) for c in comps(degc)]
+    best, best_cost = None, None
+    for egroups in ([edegs], [[d] for d in edegs]):
+        passes = []
+        for eg in egroups:
+            alist = [a for d in eg for a in comps(d)]
+            g = max(1, cmax // len(alist))
+            for i in range(0, len(clist), g):
+                tg = [(a, c) for a in alist for c in clist[i:i + g]]
+                passes.append(best_vrr(la, lb, lc, ld, tg))
+        cost = sum(p.fp64_ops() + PREAMBLE_OPS for p in passes)
+        if best is None or cost < best_cost:
+            best, best_cost = passes, cost
+    return best
+
+
+def generate_class(la, lb, lc, ld, cmax_list=()):
     tag = class_tag(la, lb, lc, ld)
     vrr = best_vrr(la, lb, lc, ld)
     hrr = HrrDag(la, lb, lc, ld)
@@ -337,24 +364,54 @@ def generate_class(la, lb, lc, ld):
     o.append(f"    static constexpr int NE = {NE}, NF = {NF}, NACC = {NE * NF}, MMAX = {vrr.max_m()};")
     o.append(f"    static constexpr int VRR_OPS = {vrr.fp64_ops()}, HRR_OPS = {hrr.fp64_ops()}, NINT = {nint};")
     o.append(f"    static constexpr bool HAS_DIAG = {'true' if diag else 'false'};")
-    o.append("    template <class Ctx>")
-    o.append("    static __device__ __forceinline__ void vrr(const Ctx &c, const double *__restrict__ F, double *__restrict__ acc) {")
+    o.append("    template <class Ctx, class Acc>")
+    o.append("    static __device__ __forceinline__ void vrr(const Ctx &c, const double *__restrict__ F, Acc &acc) {")
     vrr.emit(o)
     o.append("    }")
-    o.append("    template <class Dg>")
-    o.append("    static __device__ __forceinline__ void hrr(const double *__restrict__ acc, double ABx, double ABy, double ABz,")
+    o.append("    template <class Acc, class Dg>")
+    o.append("    static __device__ __forceinline__ void hrr(const Acc &acc, double ABx, double ABy, double ABz,")
     o.append("                                                double CDx, double CDy, double CDz, Dg &dg) {")
     hrr.emit(o)
     o.append("    }")
-    o.append("    template <class Dg>")
-    o.append("    static __device__ __forceinline__ void hrr_diag(const double *__restrict__ acc, double ABx, double ABy, double ABz,")
+    o.append("    template <class Acc, class Dg>")
+    o.append("    static __device__ __forceinline__ void hrr_diag(const Acc &acc, double ABx, double ABy, double ABz,")
     o.append("                                                     double CDx, double CDy, double CDz, Dg &dg) {")
     if diag:
         diag.emit(o)
     o.append("    }")
     o.append("};")
+    gidx = {t: i for i, t in enumerate(all_targets(la, lb, lc, ld))}
+    pass_meta = {}
+    for cmax in cmax_list:
+        passes = plan_passes(la, lb, lc, ld, cmax)
+        if len(passes) < 2:
+            continue
+        tot = sum(p.fp64_ops() for p in passes)
+        pass_meta[str(cmax)] = {"npass": len(passes), "vrr_ops": tot, "max_chunk": max(len(p.targets) for p in passes)}
+        o.append(f"// multi-pass pruned VRR, chunks of <= {cmax} accumulators: {len(passes)} passes, {tot} FP64 ops per primitive quartet")
+        o.append(f"struct GP_{tag}_{cmax} {{")
+        o.append(f"    static constexpr int NPASS = {len(passes)};")
+        o.append(f"    static constexpr int NCHUNK_MAX = {max(len(p.targets) for p in passes)};")
+        o.append("    static __host__ __device__ constexpr int pass_nacc(int P) { constexpr int t[] = {" + ", ".join(str(len(p.targets)) for p in passes) + "}; return t[P]; }")
+        o.append("    static __host__ __device__ constexpr int pass_mmax(int P) { constexpr int t[] = {" + ", ".join(str(p.max_m()) for p in passes) + "}; return t[P]; }")
+        o.append("    template <int P, class Ctx, class Acc>")
+        o.append("    static __device__ __forceinline__ void vrr_pass(const Ctx &c, const double *__restrict__ F, Acc &acc) {")
+        for k, pdag in enumerate(passes):
+            o.append(f"      if constexpr (P == {k}) {{")
+            pdag.emit(o)
+            o.append("      }")
+        o.append("    }")
+        o.append("    template <int P, class Chunk, class Acc>")
+        o.append("    static __device__ __forceinline__ void store_pass(const Chunk &ch, Acc &acc) {")
+        for k, pdag in enumerate(passes):
+            o.append(f"      if constexpr (P == {k}) {{")
+            for i, t in enumerate(pdag.targets):
+                o.append(f"        acc.template set<{gidx[t]}>(ch.template get<{i}>());")
+            o.append("      }")
+        o.append("    }")
+        o.append("};")
     meta = {"tag": tag, "l": [la, lb, lc, ld], "vrr_ops": vrr.fp64_ops(), "hrr_ops": hrr.fp64_ops(), "nint": nint,
-            "nacc": NE * NF, "vrr_nodes": len(vrr.nodes), "how": vrr.how}
+            "nacc": NE * NF, "vrr_nodes": len(vrr.nodes), "how": vrr.how, "passes": pass_meta}
     return "\n".join(o) + "\n", meta
 
 
@@ -375,15 +432,17 @@ def main():
     ap.add_argument("--out", required=True)
     ap.add_argument("--max-nacc", type=int, default=1000, help="largest NE*NF emitted as straight-line code")
     ap.add_argument("--max-l", type=int, default=2, help="highest shell l emitted as straight-line code")
+    ap.add_argument("--cmax", type=str, default="{}", help="JSON {tag: [chunk sizes]} of multi-pass variants to emit")
     args = ap.parse_args()
     os.makedirs(args.out, exist_ok=True)
+    cmax_map = json.loads(args.cmax)
     metas = []
     for (la, lb, lc, ld) in all_classes(3):
         NE = sum(ncart(e) for e in range(la, la + lb + 1))
         NF = sum(ncart(f) for f in range(lc, lc + ld + 1))
         if max(la, lb, lc, ld) > args.max_l or NE * NF > args.max_nacc:
             continue
-        src, meta = generate_class(la, lb, lc, ld)
+        src, meta = generate_class(la, lb, lc, ld, cmax_map.get(class_tag(la, lb, lc, ld), ()))
         with open(os.path.join(args.out, f"eri_{meta['tag']}.cuh"), "w") as f:
             f.write(src)
         metas.append(meta)
