@@ -24,6 +24,9 @@ struct ClassEntry {
     int la = 0, lb = 0, lc = 0, ld = 0;
     int vrr_ops = 0, hrr_ops = 0, nint = 0;   // FP64 instruction counts from the generator
     const char *impl = "none";                // "straightline" | "table"
+    const int32_t *prog = nullptr;            // host copy of the class's table program (generated/programs.bin), if any
+    int64_t prog_off = 0;                     // its offset in the blob (int32 units)
+    bool use_table = false;                   // this class runs through the interpreter kernels (adft_interp.cuh)
 };
 ClassEntry *class_table();                    // [NQCLASS]
 void register_all_classes();                  // defined in generated registry.cu

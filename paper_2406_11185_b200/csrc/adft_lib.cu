@@ -3,10 +3,12 @@
 #include <algorithm>
 #include <cfloat>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 
 #include "adft_internal.h"
+#include "adft_interp.cuh"
 
 namespace adft {
 
@@ -16,9 +18,69 @@ void set_error(const std::string &msg) { g_last_error = msg; }
 static ClassEntry g_classes[NQCLASS];
 ClassEntry *class_table() { return g_classes; }
 static bool g_registered = false;
+
+}  // namespace adft
+// table programs of every class (generated/programs.bin, linked in through generated/programs_blob.S)
+extern "C" const int32_t adft_prog_blob[];
+extern "C" const int32_t adft_prog_blob_end[];
+namespace adft {
+
+// program header fields (gen_eri.py pack_program)
+enum { PH_MAGIC = 0, PH_LA = 1, PH_LB = 2, PH_LC = 3, PH_LD = 4, PH_NVRR = 5, PH_NVSLOTS = 6, PH_NACC = 7, PH_NHRR = 8,
+       PH_NHSLOTS = 9, PH_NOUT = 10, PH_MMAX = 11, PH_VRR_OPS = 12, PH_HRR_OPS = 13, PH_NINT = 14, PH_NHRR_DIAG = 15,
+       PH_NHSLOTS_DIAG = 16, PH_NOUT_DIAG = 17, PH_OFF_VRR = 18, PH_OFF_HRR = 19, PH_OFF_DIAG = 20, PH_TOTAL = 21 };
+
 static void ensure_registered()
 {
-    if (!g_registered) { register_all_classes(); g_registered = true; }
+    if (g_registered) return;
+    register_all_classes();
+    // classes without generated straight-line code run through the interpreter; ADFT_FORCE_TABLE=1 (tests) sends
+    // every class there
+    const char *force = getenv("ADFT_FORCE_TABLE");
+    const bool force_table = force && force[0] == '1';
+    for (int qc = 0; qc < NQCLASS; ++qc) {
+        const int32_t off = adft_prog_blob[2 * qc], len = adft_prog_blob[2 * qc + 1];
+        if (len <= 0) continue;
+        const int32_t *pr = adft_prog_blob + off;
+        if (pr[PH_MAGIC] != 0x41444654 || pr[PH_TOTAL] != len) continue;
+        ClassEntry &e = g_classes[qc];
+        e.prog = pr;
+        e.prog_off = off;
+        if (!e.launch_jk || force_table) {
+            e.use_table = true;
+            e.impl = "table";
+            e.la = pr[PH_LA]; e.lb = pr[PH_LB]; e.lc = pr[PH_LC]; e.ld = pr[PH_LD];
+            e.vrr_ops = pr[PH_VRR_OPS]; e.hrr_ops = pr[PH_HRR_OPS]; e.nint = pr[PH_NINT];
+        }
+    }
+    g_registered = true;
+}
+
+static InterpProg make_prog(const ClassEntry &e, const int32_t *d_blob, bool diag)
+{
+    const int32_t *h = e.prog;
+    const int32_t *d = d_blob + e.prog_off;
+    InterpProg g{};
+    g.vrr = (const int4 *)(d + h[PH_OFF_VRR]);
+    g.hrr = (const int4 *)(d + (diag ? h[PH_OFF_DIAG] : h[PH_OFF_HRR]));
+    g.n_vrr = h[PH_NVRR];
+    g.n_hrr = diag ? h[PH_NHRR_DIAG] : h[PH_NHRR];
+    g.n_vslots = h[PH_NVSLOTS];
+    g.n_hslots = diag ? h[PH_NHSLOTS_DIAG] : h[PH_NHSLOTS];
+    g.nacc = h[PH_NACC];
+    g.mmax = h[PH_MMAX];
+    g.la = h[PH_LA]; g.lb = h[PH_LB]; g.lc = h[PH_LC]; g.ld = h[PH_LD];
+    return g;
+}
+static int jk_slots_of(const ClassEntry &e)
+{
+    const int32_t *h = e.prog;
+    return interp_jk_slots(h[PH_NVSLOTS], h[PH_NHSLOTS], h[PH_NACC], h[PH_LA], h[PH_LB], h[PH_LC], h[PH_LD]);
+}
+static int schwarz_slots_of(const ClassEntry &e)
+{
+    const int32_t *h = e.prog;
+    return h[PH_NACC] + std::max(h[PH_NVSLOTS], h[PH_NHSLOTS_DIAG]);
 }
 
 #define CUDA_TRY(expr)                                                                           \
@@ -153,6 +215,11 @@ struct adft_shellpairs {
     // staging for adft_jk_build_host
     double *d_stage = nullptr;
     size_t stage_n = 0;
+    // interpreter path (classes without straight-line code): device copy of the program blob, per-thread scratch
+    int32_t *d_blob = nullptr;
+    double *d_scratch = nullptr;
+    long long scratch_threads = 0;     // threads of the persistent interpreter grid = scratch stride
+    int interp_blocks = 0;
     // sink for the output the caller skipped (J == NULL or K == NULL): round 1 has one kernel variant per class
     double *d_sink = nullptr;
 };
@@ -287,6 +354,7 @@ static void free_pairs(adft_shellpairs *p)
     cudaFree(p->d_xyz); cudaFree(p->d_expo); cudaFree(p->d_coef); cudaFree(p->d_atom); cudaFree(p->d_nprim);
     cudaFree(p->d_off); cudaFree(p->d_Q); cudaFree(p->d_AB); cudaFree(p->d_prim); cudaFree(p->d_pint);
     cudaFree(p->d_boys); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage); cudaFree(p->d_sink);
+    cudaFree(p->d_blob); cudaFree(p->d_scratch);
     if (p->h_segs) cudaFreeHost(p->h_segs);
     if (p->h_small) cudaFreeHost(p->h_small);
     if (p->ev_ok) for (auto &e : p->ev) cudaEventDestroy(e);
@@ -395,7 +463,7 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
     // every needed Schwarz class must exist
     for (const Sublist &s : p->subl) {
         const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
-        if (!ce.launch_schwarz) {
+        if (!ce.launch_schwarz && !ce.prog) {
             set_error("adft_shellpairs_build: no kernel for pair class (" + std::to_string(s.la) + "," + std::to_string(s.lb) + ")");
             free_pairs(p); return ADFT_ERR_UNSUPPORTED_L;
         }
@@ -418,7 +486,27 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
     ALLOC(p->d_pint, 4 * np * sizeof(int32_t));
     ALLOC(p->d_prim, 9 * npp * sizeof(double));
     ALLOC(p->d_boys, (size_t)BOYS_NT * BOYS_NM * sizeof(double));
-    ALLOC(p->d_counters, 2 * NQCLASS * sizeof(unsigned long long));
+    ALLOC(p->d_counters, 3 * NQCLASS * sizeof(unsigned long long));
+    {
+        // interpreter resources, only if some class that can occur lacks straight-line code
+        int slots = 0;
+        for (int X = 0; X < NPAIRCLASS; ++X)
+            for (int Y = 0; Y <= X; ++Y) {
+                if (p->subl_of_class[X].empty() || p->subl_of_class[Y].empty()) continue;
+                const ClassEntry &ce = class_table()[quartet_class(X, Y)];
+                if (ce.use_table) slots = std::max(slots, jk_slots_of(ce));
+                if (X == Y && (ce.use_table || !ce.launch_schwarz)) slots = std::max(slots, schwarz_slots_of(ce));
+            }
+        if (slots > 0) {
+            int dev = 0, sms = 0;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            p->interp_blocks = sms * 4;
+            p->scratch_threads = (long long)p->interp_blocks * 128;
+            ALLOC(p->d_blob, (size_t)(adft_prog_blob_end - adft_prog_blob) * sizeof(int32_t));
+            ALLOC(p->d_scratch, (size_t)slots * (size_t)p->scratch_threads * sizeof(double));
+        }
+    }
     ALLOC(p->d_dmax, 2 * sizeof(unsigned long long));
 #undef ALLOC
     if (cudaMallocHost((void **)&p->h_small, 4 * NQCLASS * sizeof(unsigned long long)) != cudaSuccess) {
@@ -445,6 +533,9 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
     TRY2(cudaMemcpyAsync(p->d_atom, b->atom.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     TRY2(cudaMemcpyAsync(p->d_nprim, b->nprimv.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     TRY2(cudaMemcpyAsync(p->d_off, b->off.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    if (p->d_blob)
+        TRY2(cudaMemcpyAsync(p->d_blob, adft_prog_blob, (size_t)(adft_prog_blob_end - adft_prog_blob) * sizeof(int32_t),
+                             cudaMemcpyHostToDevice, st));
     std::vector<double> boys;
     fill_boys_table(boys);
     TRY2(cudaMemcpyAsync(p->d_boys, boys.data(), boys.size() * sizeof(double), cudaMemcpyHostToDevice, st));
@@ -455,7 +546,18 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
     if (rc) return fail(rc);
     for (const Sublist &s : p->subl) {
         if (s.n == 0) continue;
-        class_table()[quartet_class(s.pc, s.pc)].launch_schwarz(p->tab, s.pair_base, s.prim_base, s.n, s.K, p->d_boys, p->d_Q, st);
+        const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
+        if (ce.launch_schwarz && !ce.use_table) {
+            ce.launch_schwarz(p->tab, s.pair_base, s.prim_base, s.n, s.K, p->d_boys, p->d_Q, st);
+        } else {
+            const InterpProg pg = make_prog(ce, p->d_blob, true);
+            for (long long first = 0; first < s.n; first += p->scratch_threads) {
+                const int count = (int)std::min<long long>(p->scratch_threads, s.n - first);
+                schwarz_interp_kernel<<<(count + 127) / 128, 128, 0, st>>>(p->tab, pg, s.pair_base, s.prim_base, s.n, s.K,
+                                                                          (int)first, count, p->d_boys, p->d_Q,
+                                                                          p->d_scratch, p->scratch_threads);
+            }
+        }
     }
     TRY2(cudaGetLastError());
     std::vector<double> Q(np);
@@ -556,7 +658,8 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
     // every class that can occur must have a kernel
     for (int X = 0; X < NPAIRCLASS; ++X)
         for (int Y = 0; Y <= X; ++Y)
-            if (!p->subl_of_class[X].empty() && !p->subl_of_class[Y].empty() && !class_table()[quartet_class(X, Y)].launch_jk) {
+            if (!p->subl_of_class[X].empty() && !p->subl_of_class[Y].empty() && !class_table()[quartet_class(X, Y)].launch_jk &&
+                !class_table()[quartet_class(X, Y)].use_table) {
                 set_error("adft_jk_build: no kernel compiled for quartet class " + std::to_string(quartet_class(X, Y)));
                 return ADFT_ERR_UNSUPPORTED_L;
             }
@@ -604,7 +707,7 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         }
         if (o) CUDA_TRY(cudaMemcpyAsync(p->d_segs, p->h_segs, o * sizeof(Segment), cudaMemcpyHostToDevice, st));
     }
-    CUDA_TRY(cudaMemsetAsync(p->d_counters, 0, 2 * NQCLASS * sizeof(unsigned long long), st));
+    CUDA_TRY(cudaMemsetAsync(p->d_counters, 0, 3 * NQCLASS * sizeof(unsigned long long), st));
     if (J) CUDA_TRY(cudaMemsetAsync(J, 0, n2 * sizeof(double), st));
     if (K) CUDA_TRY(cudaMemsetAsync(K, 0, n2 * sizeof(double), st));
     CUDA_TRY(cudaEventRecord(ev_plan, st));
@@ -622,7 +725,18 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         prm.D = D; prm.J = Jw; prm.K = Kw; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boys;
         prm.counters = p->d_counters + 2 * qc; prm.zero = 0;
         CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
-        class_table()[qc].launch_jk(prm, st, J != nullptr, K != nullptr); ++launches;
+        const ClassEntry &ce = class_table()[qc];
+        if (ce.use_table) {
+            InterpParams ip{};
+            ip.jk = prm; ip.prog = make_prog(ce, p->d_blob, false);
+            ip.scratch = p->d_scratch; ip.stride = p->scratch_threads;
+            ip.tile_counter = p->d_counters + 2 * NQCLASS + qc;
+            const long long want = (warps[qc] + 3) / 4;
+            jk_interp_kernel<<<(unsigned)std::min<long long>(want, p->interp_blocks), 128, 0, st>>>(ip);
+        } else {
+            ce.launch_jk(prm, st, J != nullptr, K != nullptr);
+        }
+        ++launches;
         CUDA_TRY(cudaEventRecord(ev[2 * qc + 1], st));
         p->class_ran[qc] = true;
     }

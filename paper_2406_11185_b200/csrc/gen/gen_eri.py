@@ -457,22 +457,21 @@ def main():
     print(f"generated {len(metas)} classes into {args.out}")
 
 
-if __name__ == "__main__":
-    main()
-
-
 # ----------------------------------------------------------------------------------------------------------------
 # Table programs for the interpreter kernels (classes too large for straight-line code: everything with an f shell).
 # The same DAGs as above are serialised as int32 instruction lists; value slots are assigned by liveness (linear scan)
 # so that the per-thread scratch stays small.  Layout (little-endian int32):
 #   header[32]: magic 0x41444654, la, lb, lc, ld, n_vrr, n_vslots, nacc, n_hrr, n_hslots, n_out, mmax, vrr_ops, hrr_ops,
-#               nint, n_hrr_diag, n_hslots_diag, n_out_diag, 0...
+#               nint, n_hrr_diag, n_hslots_diag, n_out_diag, off_vrr, off_hrr, off_hrr_diag, total_len, 0...
+#               (offsets and lengths in int32 units from the start of the program)
 #   vrr[n_vrr][8]:  kind | dir<<4, dst, s0, s1, s2, s3, n2, nx      kind: 0 B (s0 = m), 1 T(bra), 2 T(ket), 3 A, 4 K,
 #                   5 ACC (acc[n2] += v[s0]);  unused operands are -1
-#   hrr[n_hrr][4]:  which | dir<<1 (which: 0 AB, 1 CD), dst, k0, k1  with h = v[k0] + G_dir * v[k1];
-#                   operands >= 0 are h slots, operands < 0 are accumulators -(1+index)
-#   out[n_out][5]:  ia, ib, ic, id, src (same operand encoding)
-#   then the same three arrays' diag variants (hrr_diag, out_diag) for classes (ab|ab)
+#   hrr[n_hrr][4]:  which | dir<<2 (which: 0 AB, 1 CD), dst, k0, k1  with h[dst] = v(k0) + G_dir * v(k1);
+#                   operands >= 0 are h slots, operands < 0 are accumulators -(1+index);
+#                   which = 2 is an OUTPUT record: dst = ia | ib<<8 | ic<<16 | id<<24, k0 = the integral's operand
+#                   (outputs are interleaved with the recurrences in execution order; n_hrr counts both)
+#   hrr_diag:       the same for the diagonal integrals (mu nu|mu nu) of classes (ab|ab) (Schwarz bound)
+#   every list is followed by one all-zero pad instruction (the interpreter prefetches one ahead)
 import struct
 
 K_B, K_TBRA, K_TKET, K_A, K_K, K_ACC = 0, 1, 2, 3, 4, 5
@@ -587,7 +586,8 @@ def hrr_program(hdag):
     return ins, len(steps), n, sum(1 for t, _ in steps if t == "o")
 
 
-def write_program(path, la, lb, lc, ld):
+def pack_program(la, lb, lc, ld):
+    """int32 list of one class program (layout above) plus its meta dict."""
     vrr = best_vrr(la, lb, lc, ld)
     hrr = HrrDag(la, lb, lc, ld)
     vins, nv, nvs = vrr_program(vrr)
@@ -597,14 +597,49 @@ def write_program(path, la, lb, lc, ld):
     else:
         dins, ndh, ndhs, ndout = [], 0, 0, 0
     nint = ncart(la) * ncart(lb) * ncart(lc) * ncart(ld)
+    # every list is padded by one all-zero instruction: the interpreter prefetches instruction i+1 while executing i
+    vins = vins + [0] * 8
+    hins = hins + [0] * 4
+    dins = dins + [0] * 4
+    off_v = 32
+    off_h = off_v + len(vins)
+    off_d = off_h + len(hins)
+    total = off_d + len(dins)
     header = [0x41444654, la, lb, lc, ld, nv, nvs, len(vrr.targets), nh, nhs, nout, vrr.max_m(), vrr.fp64_ops(),
-              hrr.fp64_ops(), nint, ndh, ndhs, ndout]
+              hrr.fp64_ops(), nint, ndh, ndhs, ndout, off_v, off_h, off_d, total]
     header += [0] * (32 - len(header))
-    data = header + vins + hins + dins
+    meta = {"tag": class_tag(la, lb, lc, ld), "l": [la, lb, lc, ld], "vrr_ops": vrr.fp64_ops(), "hrr_ops": hrr.fp64_ops(),
+            "nint": nint, "nacc": len(vrr.targets), "n_vrr": nv, "n_vslots": nvs, "n_hrr": nh, "n_hslots": nhs,
+            "how": vrr.how}
+    return header + vins + hins + dins, meta
+
+
+def write_program(path, la, lb, lc, ld):
+    data, meta = pack_program(la, lb, lc, ld)
     with open(path, "wb") as f:
         f.write(struct.pack("<%di" % len(data), *data))
-    return {"tag": class_tag(la, lb, lc, ld), "l": [la, lb, lc, ld], "vrr_ops": vrr.fp64_ops(), "hrr_ops": hrr.fp64_ops(),
-            "nint": nint, "nacc": len(vrr.targets), "n_vrr": nv, "n_vslots": nvs, "n_hrr": nh, "n_hslots": nhs}
+    return meta
+
+
+def write_blob(path, classes):
+    """All class programs in one file: int32 dir[56][2] = (offset, length) in int32 units indexed by quartet class
+    qc = X(X+1)/2+Y (X >= Y pair classes, pc = la(la+1)/2+lb), zero if absent; then the programs (16-byte aligned)."""
+    ndir = 56
+    directory = [0] * (2 * ndir)
+    body, metas = [], []
+    for (la, lb, lc, ld) in classes:
+        data, meta = pack_program(la, lb, lc, ld)
+        X, Y = la * (la + 1) // 2 + lb, lc * (lc + 1) // 2 + ld
+        qc = X * (X + 1) // 2 + Y
+        assert len(data) % 4 == 0
+        directory[2 * qc] = 2 * ndir + len(body)
+        directory[2 * qc + 1] = len(data)
+        body += data
+        metas.append(meta)
+    data = directory + body
+    with open(path, "wb") as f:
+        f.write(struct.pack("<%di" % len(data), *data))
+    return metas
 
 
 def eval_program(path, ctx, AB, CD, diag=False):
@@ -614,9 +649,11 @@ def eval_program(path, ctx, AB, CD, diag=False):
     assert d[0] == 0x41444654
     la, lb, lc, ld, nv, nvs, nacc, nh, nhs, nout, mmax = d[1:12]
     ndh, ndhs, ndout = d[15:18]
+    off_v, off_h, off_d, total = d[18:22]
+    assert total == len(d)
     v = [0.0] * max(nvs, 1)
     acc = [0.0] * nacc
-    p = 32
+    p = off_v
     for i in range(nv):
         op, dst, s0, s1, s2, s3, n2, nx = d[p:p + 8]; p += 8
         kind, dr = op & 15, (op >> 4) & 3
@@ -640,8 +677,9 @@ def eval_program(path, ctx, AB, CD, diag=False):
             v[dst] = x
         else:
             acc[n2] += v[s0]
+    p = off_h
     if diag:
-        p += 4 * nh
+        p = off_d
         nh, nhs = ndh, ndhs
     h = [0.0] * max(nhs, 1)
     rd = lambda k: acc[-k - 1] if k < 0 else h[k]
@@ -654,3 +692,7 @@ def eval_program(path, ctx, AB, CD, diag=False):
         else:
             h[dst] = rd(k0) + (AB if which == 0 else CD)[dr] * rd(k1)
     return out
+
+
+if __name__ == "__main__":
+    main()

@@ -82,7 +82,21 @@ def test_class_sweep_all_orderings(api, orc, chunk):
         check_full(api, orc, w, tau=0.0)
 
 
-@pytest.mark.parametrize("ls", [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (2, 2), (0, 2), (1, 2)])
+F_COMBOS = [c for c in itertools.product([0, 1, 2, 3], repeat=4) if 3 in c]        # 175 ordered combinations with an f shell
+
+
+@pytest.mark.parametrize("chunk", range(7))
+def test_class_sweep_f_orderings(api, orc, chunk):
+    """The same sweep for every ordered (la,lb,lc,ld) that contains an f shell (all 34 f classes, both orientations)."""
+    atoms = np.array([[0.0, 0.1, -0.2], [1.3, -0.4, 0.5], [-0.6, 1.1, 0.9], [0.7, 0.8, -1.2]])
+    for ls in F_COMBOS[chunk * 25:(chunk + 1) * 25]:
+        w = W.make_custom(atoms, [(i, ls[i]) for i in range(4)], seed=3000 + sum(l * 4 ** i for i, l in enumerate(ls)),
+                          emin=0.2, emax=8.0)
+        check_full(api, orc, w, tau=0.0)
+
+
+@pytest.mark.parametrize("ls", [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (2, 2), (0, 2), (1, 2),
+                                (3, 0), (3, 1), (3, 2), (3, 3), (0, 3), (2, 3)])
 def test_coincident_shells(api, orc, ls):
     """Two shells on ONE atom and a copy of them on a second: exercises A=B, C=D, AB=CD weights and AB=0 geometry."""
     atoms = np.array([[0.0, 0.0, 0.0], [0.9, -0.7, 1.1]])
@@ -90,6 +104,21 @@ def test_coincident_shells(api, orc, ls):
     w = W.make_custom(atoms, spec, seed=500 + 10 * ls[0] + ls[1], emin=0.2, emax=8.0)
     check_full(api, orc, w, tau=0.0)
     check_full(api, orc, w, tau=1e-6)
+
+
+def test_interpreter_on_all_low_classes():
+    """ADFT_FORCE_TABLE=1 sends every class through the table interpreter (adft_interp.cuh); the s/p/d parity cases
+    must pass there too (the switch is read once per process, hence the subprocess)."""
+    import os
+    import subprocess
+    import sys
+    if os.environ.get("ADFT_FORCE_TABLE") == "1":
+        pytest.skip("already inside the forced-table run")
+    env = dict(os.environ, ADFT_FORCE_TABLE="1")
+    r = subprocess.run([sys.executable, "-m", "pytest", __file__, "-q", "-x", "-m", "gpu", "-k",
+                        "config_full_parity or cfg1_unscreened or class_sweep_all_orderings or j_only_k_only"],
+                       env=env, capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-2000:]
 
 
 def test_j_only_k_only_and_repeat(api, orc):
@@ -175,3 +204,8 @@ def sampled_parity(api, orc, w, nsamples, seed):
 
 def test_cfg2_sampled_parity(api, orc):
     sampled_parity(api, orc, W.make(2), nsamples=6, seed=2)
+
+
+def test_cfg3_sampled_parity(api, orc):
+    """cfg 3 (f shells on the heavy atoms, d on the light ones): all 55 quartet classes."""
+    sampled_parity(api, orc, W.make(3), nsamples=4, seed=3)
