@@ -145,6 +145,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--prim-threshold", type=float, default=None,
+                    help="primitive-pair threshold (default: the library's ADFT_DEFAULT_PRIM_THRESHOLD; 0 = no primitive screening)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -172,10 +174,11 @@ def main():
     N = w.nbf
     t0 = time.perf_counter()
     bs = api.Basis.from_workload(w)
-    sp = api.ShellPairs(bs)
+    sp = api.ShellPairs(bs, prim_threshold=args.prim_threshold)
     torch.cuda.synchronize()
     t_pairs = time.perf_counter() - t0
     npairs, nprimpairs = sp.counts()
+    nprim_nominal, _, prim_thr = sp.prim_counts()
     D = torch.from_numpy(w.D).cuda()
     J = torch.empty_like(D); K = torch.empty_like(D)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
@@ -257,14 +260,19 @@ def main():
                "config": {"workload": WORKLOAD_NAMES[args.config], "nbf": N, "nshells": w.nshells, "natoms": w.natoms,
                           "tau": w.tau, "shell_pairs": npairs, "primitive_pairs": nprimpairs,
                           "quartets_unique": int(stats.quartets_unique), "quartets_kept": kept,
-                          "prim_quartets": int(stats.prim_quartets), "parallelism": "replicas" if world > 1 else "1gpu",
+                          "primitive_pairs_nominal": nprim_nominal, "prim_threshold": prim_thr,
+                          "prim_quartets": int(stats.prim_quartets),
+                          "prim_quartets_evaluated": int(stats.prim_quartets_evaluated), "parallelism": "replicas" if world > 1 else "1gpu",
                           "l2": "flushed between iterations (256 MiB write); pair table + D/J/K exceed L2",
                           "shellpairs_build_s": t_pairs},
                "jk_build_ms": ms_step, "region_ms": region_ms,
                "prim_quartets_per_s": world * int(stats.prim_quartets) / (ms_step * 1e-3),
+               "prim_quartets_evaluated_per_s": world * int(stats.prim_quartets_evaluated) / (ms_step * 1e-3),
                "model_tflops": step_tflops, "fp64_peak_fraction": step_tflops / peak,
                "phase_ms": {"dmax": stats.ms_dmax, "plan": stats.ms_plan, "eri": stats.ms_eri, "finalize": stats.ms_finalize},
                "class_ms": {CLASS_NAMES[i]: round(float(class_ms[i]), 3) for i in range(55) if cq[i]},
+               "class_model_tflops": {CLASS_NAMES[i]: round(float(cmf[i] / (class_ms[i] * 1e-3) / 1e12), 2)
+                                      for i in range(55) if cq[i] and class_ms[i] > 0},
                "roofline": roofline,
                "e2e": {"value": e2e_value, "unit": "quartets/s", "ms_per_step": e2e_ms,
                        "h2d_bytes_per_step": int(N) * N * 8, "d2h_bytes_per_step": 2 * int(N) * N * 8},

@@ -65,9 +65,11 @@ typedef struct adft_shellpairs adft_shellpairs_t; /* opaque; owns every device w
 typedef struct {
     int64_t quartets_unique;      /* unique shell quartets before screening = P(P+1)/2 */
     int64_t quartets_kept;        /* unique shell quartets that pass the screen (the metric's numerator) */
-    int64_t prim_quartets;        /* primitive quartets inside the kept quartets */
+    int64_t prim_quartets;        /* primitive quartets inside the kept quartets, nominal (full contraction depth) */
+    int64_t prim_quartets_evaluated; /* primitive quartets actually evaluated (after primitive-pair screening) */
     int64_t class_quartets[ADFT_MAX_CLASSES]; /* kept per class; class = X(X+1)/2+Y, X >= Y pair classes,
                                                  pair class = hi(hi+1)/2+lo of the two angular momenta */
+    int64_t class_prim_quartets[ADFT_MAX_CLASSES]; /* evaluated primitive quartets per class */
     double  class_ms[ADFT_MAX_CLASSES];       /* device time of each class kernel (CUDA events) */
     double  class_model_flops[ADFT_MAX_CLASSES]; /* model FP64 flops of each class launch */
     double  model_flops;          /* FP64 flops of the generated recurrences for the kept work */
@@ -101,6 +103,21 @@ adft_status_t adft_basis_coefficients(const adft_basis_t *basis, double *coeffic
  * descending inside a bucket.  Work is enqueued on cuda_stream (a cudaStream_t, may be NULL = default stream) and the
  * call synchronises that stream before returning.  The basis must outlive the pairs handle. */
 adft_status_t adft_shellpairs_build(const adft_basis_t *basis, void *cuda_stream, adft_shellpairs_t **out);
+
+/* The same with an explicit primitive-pair threshold (reading R-11; the paper is silent on primitive
+ * screening).  After the Schwarz bounds have been computed from the FULL contraction, a primitive pair (i on A, j on B)
+ * is dropped from the table when its estimated primitive Schwarz factor
+ *   sqrt|(ij|ij)| ~ |d_i d_j| exp(-a b |AB|^2/(a+b)) sqrt(2 pi^(5/2)/((a+b)^2 sqrt(2(a+b)))) (|PA|+(a+b)^-1/2)^la (|PB|+(a+b)^-1/2)^lb
+ * is below prim_threshold (absolute, in sqrt(Hartree)); the largest primitive pair of a shell pair is always kept.
+ * prim_threshold = 0 keeps every primitive pair (the plain definition, what the oracle evaluates).
+ * adft_shellpairs_build uses ADFT_DEFAULT_PRIM_THRESHOLD.  Errors: negative or non-finite threshold -> INVALID_ARG. */
+#define ADFT_DEFAULT_PRIM_THRESHOLD 1e-20
+adft_status_t adft_shellpairs_build_ex(const adft_basis_t *basis, double prim_threshold, void *cuda_stream,
+                                       adft_shellpairs_t **out);
+
+/* Primitive-pair records before / after primitive screening and the threshold used. */
+adft_status_t adft_shellpairs_prim_counts(const adft_shellpairs_t *pairs, int64_t *nominal, int64_t *kept,
+                                          double *threshold);
 
 /* Schwarz bounds as a full symmetric HOST matrix Q[nshells*nshells] (row-major, shell order of the basis). */
 adft_status_t adft_shellpairs_schwarz(const adft_shellpairs_t *pairs, double *Q);

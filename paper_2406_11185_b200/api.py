@@ -31,7 +31,9 @@ class AdftError(RuntimeError):
 
 class JKStats(C.Structure):
     _fields_ = [("quartets_unique", C.c_int64), ("quartets_kept", C.c_int64), ("prim_quartets", C.c_int64),
-                ("class_quartets", C.c_int64 * ADFT_MAX_CLASSES), ("class_ms", C.c_double * ADFT_MAX_CLASSES),
+                ("prim_quartets_evaluated", C.c_int64),
+                ("class_quartets", C.c_int64 * ADFT_MAX_CLASSES),
+                ("class_prim_quartets", C.c_int64 * ADFT_MAX_CLASSES), ("class_ms", C.c_double * ADFT_MAX_CLASSES),
                 ("class_model_flops", C.c_double * ADFT_MAX_CLASSES),
                 ("model_flops", C.c_double), ("dmax", C.c_double),
                 ("ms_dmax", C.c_double), ("ms_plan", C.c_double), ("ms_eri", C.c_double),
@@ -40,7 +42,7 @@ class JKStats(C.Structure):
 
 
 EXPORTS = ["adft_basis_create", "adft_basis_nbf", "adft_basis_shell_offsets", "adft_basis_coefficients",
-           "adft_shellpairs_build", "adft_shellpairs_schwarz", "adft_jk_build", "adft_jk_build_host", "adft_jk_stats",
+           "adft_shellpairs_build", "adft_shellpairs_build_ex", "adft_shellpairs_prim_counts", "adft_shellpairs_schwarz", "adft_jk_build", "adft_jk_build_host", "adft_jk_stats",
            "adft_shellpairs_counts", "adft_shellpairs_destroy", "adft_basis_destroy", "adft_status_string",
            "adft_last_error", "adft_fp64_peak_tflops"]
 
@@ -59,6 +61,7 @@ def lib():
         L.adft_jk_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.adft_jk_build_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.adft_shellpairs_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.adft_shellpairs_build_ex.argtypes = [C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
         L.adft_jk_stats.argtypes = [C.c_void_p, C.c_void_p]
         L.adft_fp64_peak_tflops.argtypes = [C.c_void_p, C.c_void_p]
         _lib = L
@@ -128,10 +131,19 @@ class Basis:
 class ShellPairs:
     """adft_shellpairs_build + adft_jk_build on torch CUDA tensors."""
 
-    def __init__(self, basis: Basis, stream=None):
+    def __init__(self, basis: Basis, stream=None, prim_threshold=None):
         self.basis = basis
         self._h = C.c_void_p()
-        _check(lib().adft_shellpairs_build(basis._h, _stream_ptr(stream), C.byref(self._h)))
+        if prim_threshold is None:
+            _check(lib().adft_shellpairs_build(basis._h, _stream_ptr(stream), C.byref(self._h)))
+        else:
+            _check(lib().adft_shellpairs_build_ex(basis._h, C.c_double(prim_threshold), _stream_ptr(stream),
+                                                  C.byref(self._h)))
+
+    def prim_counts(self):
+        a, b, t = C.c_int64(), C.c_int64(), C.c_double()
+        _check(lib().adft_shellpairs_prim_counts(self._h, C.byref(a), C.byref(b), C.byref(t)))
+        return int(a.value), int(b.value), float(t.value)
 
     def schwarz(self):
         Q = np.zeros((self.basis.nshells, self.basis.nshells), np.float64)
@@ -185,11 +197,11 @@ def fp64_peak_tflops(stream=None) -> float:
     return float(v.value)
 
 
-def jk(workload, tau=None, want_j=True, want_k=True):
+def jk(workload, tau=None, want_j=True, want_k=True, prim_threshold=None):
     """Convenience: full path on cuda:0 for a workloads.Workload; returns numpy J, K and the stats."""
     import torch
     bs = Basis.from_workload(workload)
-    sp = ShellPairs(bs)
+    sp = ShellPairs(bs, prim_threshold=prim_threshold)
     D = torch.from_numpy(workload.D).cuda()
     J = torch.empty_like(D) if want_j else None
     K = torch.empty_like(D) if want_k else None

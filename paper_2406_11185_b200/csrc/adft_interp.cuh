@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(128) jk_interp_kernel(const InterpParams q)
            *dad = dac + (long long)na * nc * st, *dbc = dad + (long long)na * nd * st, *dbd = dbc + (long long)nb * nc * st;
     double *jab = dbd + (long long)nb * nd * st, *jcd = jab + (long long)na * nb * st, *kac = jcd + (long long)nc * nd * st,
            *kad = kac + (long long)na * nc * st, *kbc = kad + (long long)na * nd * st, *kbd = kbc + (long long)nb * nc * st;
-    unsigned long long cnt_q = 0ull, cnt_p = 0ull;
+    unsigned long long cnt_q = 0ull, cnt_p = 0ull, cnt_n = 0ull;
     for (;;) {
         long long w = 0;
         if (lane == 0) w = (long long)atomicAdd(q.tile_counter, 1ull);
@@ -158,10 +158,12 @@ __global__ void __launch_bounds__(128) jk_interp_kernel(const InterpParams q)
         valid = valid && ((Qab * __ldg(p.t.Q + gcd)) * p.dmax >= p.tau);      // the screen (DESIGN R-7)
         const unsigned ballot = __ballot_sync(0xffffffffu, valid);
         if (ballot == 0u) continue;
+        const unsigned knom_cd = __reduce_add_sync(0xffffffffu, valid ? (unsigned)__ldg(p.t.knom + gcd) : 0u);
         if (lane == 0) {
             const unsigned long long n = (unsigned long long)__popc(ballot);
             cnt_q += n;
             cnt_p += n * (unsigned long long)(sg.bra_K * sg.ket_K);
+            cnt_n += (unsigned long long)__ldg(p.t.knom + gab) * knom_cd;
         }
         for (int x = 0; x < pg.nacc; ++x) A[x * st] = 0.0;
         for (int kb = 0; kb < sg.bra_K; ++kb) {
@@ -231,6 +233,7 @@ __global__ void __launch_bounds__(128) jk_interp_kernel(const InterpParams q)
     if (lane == 0 && cnt_q) {
         atomicAdd(p.counters, cnt_q);
         atomicAdd(p.counters + 1, cnt_p);
+        atomicAdd(p.counters + 2, cnt_n);
     }
 }
 

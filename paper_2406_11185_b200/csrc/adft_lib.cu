@@ -95,8 +95,30 @@ static int schwarz_slots_of(const ClassEntry &e)
 static inline int ncart(int l) { return (l + 1) * (l + 2) / 2; }
 
 // ------------------------------------------------------------------ small kernels
-// (a2) primitive-pair records of one sublist (all pairs share la, lb and K = npa*npb).
-__global__ void pair_prim_kernel(int pair_base, int prim_base, int n, const int32_t *__restrict__ sha,
+// (a2) primitive screening estimate of primitive pair (alpha on A, beta on B) of a shell pair with angular momenta
+// (la, lb): the primitive Schwarz factor sqrt|(ij|ij)|.  For s functions it is exact,
+//   sqrt( 2 pi^(5/2) / (zeta^2 sqrt(2 zeta)) ) |d_a d_b| exp(-alpha beta |AB|^2 / zeta);
+// for l > 0 every Cartesian factor (x - A_x) is bounded on the support of the product Gaussian by
+// |P - A| + 1/sqrt(zeta) (distance of the product centre plus its width).  DESIGN.md reading R-11.
+__device__ __forceinline__ double prim_pair_estimate(double a, double b, double da, double db, double AB2, int la, int lb)
+{
+    const double z = a + b, iz = 1.0 / z;
+    const double w = sqrt(iz);
+    const double rAB = sqrt(AB2);
+    const double pa = b * iz * rAB + w, pb = a * iz * rAB + w;       // |P-A| + width, |P-B| + width
+    double f = fabs(da * db) * exp(-a * b * iz * AB2) * sqrt(34.986836655249725 * iz * iz * sqrt(0.5 * iz));  // 2 pi^2.5
+    for (int i = 0; i < la; ++i) f *= pa;
+    for (int i = 0; i < lb; ++i) f *= pb;
+    return f;
+}
+
+// (a2) primitive-pair records of one sublist.  Two modes:
+//   kcount != NULL : count, per pair, the primitive pairs whose estimate is >= thr (at least 1: the largest is always
+//                    kept) and write the count to kcount[g]; no records are written;
+//   kcount == NULL : write the records of the surviving primitive pairs (the same rule, same arithmetic) in nominal
+//                    order (ia major, ib minor) to slots k = 0..K-1 of the sublist (all its pairs have K survivors).
+__global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int la, int lb, double thr, int32_t *kcount,
+                                 const int32_t *__restrict__ sha,
                                  const int32_t *__restrict__ shb, const int32_t *__restrict__ sh_atom,
                                  const int32_t *__restrict__ sh_nprim, const int32_t *__restrict__ sh_off,
                                  const double *__restrict__ xyz, const double *__restrict__ expo,
@@ -111,17 +133,32 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, const int3
     const double Bx = xyz[3 * sh_atom[sb]], By = xyz[3 * sh_atom[sb] + 1], Bz = xyz[3 * sh_atom[sb] + 2];
     const double AB2 = (Ax - Bx) * (Ax - Bx) + (Ay - By) * (Ay - By) + (Az - Bz) * (Az - Bz);
     const int npa = sh_nprim[sa], npb = sh_nprim[sb];
+    int cnt = 0, best = 0;
+    double best_est = -1.0;
+    for (int ia = 0; ia < npa; ++ia)
+        for (int ib = 0; ib < npb; ++ib) {
+            const double est = prim_pair_estimate(expo[sh_off[sa] + ia], expo[sh_off[sb] + ib], coef[sh_off[sa] + ia],
+                                                  coef[sh_off[sb] + ib], AB2, la, lb);
+            if (est >= thr) ++cnt;
+            if (est > best_est) { best_est = est; best = ia * npb + ib; }
+        }
+    if (kcount) { kcount[g] = cnt > 0 ? cnt : 1; return; }
     const double c0 = 5.9149671727956128778;     // sqrt(2) * pi^(5/4)
+    int k = 0;
     for (int ia = 0; ia < npa; ++ia)
         for (int ib = 0; ib < npb; ++ib) {
             const double a = expo[sh_off[sa] + ia], b = expo[sh_off[sb] + ib];
+            const double da = coef[sh_off[sa] + ia], db = coef[sh_off[sb] + ib];
+            const bool keep = cnt > 0 ? (prim_pair_estimate(a, b, da, db, AB2, la, lb) >= thr) : (ia * npb + ib == best);
+            if (!keep) continue;
             const double z = a + b, iz = 1.0 / z;
             const double px = (a * Ax + b * Bx) * iz, py = (a * Ay + b * By) * iz, pz = (a * Az + b * Bz) * iz;
-            const int idx = prim_base + (ia * npb + ib) * n + j;
+            const int idx = prim_base + k * n + j;
             zeta[idx] = z;  inv2z[idx] = 0.5 * iz;
             Px[idx] = px;  Py[idx] = py;  Pz[idx] = pz;
             PAx[idx] = px - Ax;  PAy[idx] = py - Ay;  PAz[idx] = pz - Az;
-            cc[idx] = c0 * coef[sh_off[sa] + ia] * coef[sh_off[sb] + ib] * exp(-a * b * iz * AB2) * iz;
+            cc[idx] = c0 * da * db * exp(-a * b * iz * AB2) * iz;
+            ++k;
         }
 }
 
@@ -188,7 +225,8 @@ struct Sublist {
 
 struct adft_shellpairs {
     const adft_basis *basis = nullptr;
-    int64_t npairs = 0, nprimpairs = 0;
+    int64_t npairs = 0, nprimpairs = 0, nprimpairs_nominal = 0;
+    double prim_threshold = 0.0;
     std::vector<Sublist> subl;
     std::vector<int> subl_of_class[NPAIRCLASS];
     std::vector<double> hQ;            // sorted order
@@ -198,7 +236,7 @@ struct adft_shellpairs {
     int32_t *d_atom = nullptr, *d_nprim = nullptr, *d_off = nullptr;
     // device: pair table
     double *d_Q = nullptr, *d_AB = nullptr /* 3*npairs */, *d_prim = nullptr /* 9*nprimpairs */;
-    int32_t *d_pint = nullptr /* 4*npairs: bfa,bfb,sha,shb */;
+    int32_t *d_pint = nullptr /* 5*npairs: bfa,bfb,sha,shb,knom */;
     double *d_boys = nullptr;
     PairTable tab{};
     // per-build workspaces
@@ -362,7 +400,7 @@ static void free_pairs(adft_shellpairs *p)
 }
 extern "C" void adft_shellpairs_destroy(adft_shellpairs_t *p) { free_pairs(p); }
 
-struct HostPair { int sa, sb; double Q; };
+struct HostPair { int sa, sb; double Q; int knom; };
 
 static void set_table_pointers(adft_shellpairs *p)
 {
@@ -371,21 +409,23 @@ static void set_table_pointers(adft_shellpairs *p)
     t.Q = p->d_Q;
     t.ABx = p->d_AB; t.ABy = p->d_AB + np; t.ABz = p->d_AB + 2 * np;
     t.bfa = p->d_pint; t.bfb = p->d_pint + np; t.sha = p->d_pint + 2 * np; t.shb = p->d_pint + 3 * np;
+    t.knom = p->d_pint + 4 * np;
     t.zeta = p->d_prim; t.inv2z = p->d_prim + npp; t.Px = p->d_prim + 2 * npp; t.Py = p->d_prim + 3 * npp;
     t.Pz = p->d_prim + 4 * npp; t.PAx = p->d_prim + 5 * npp; t.PAy = p->d_prim + 6 * npp; t.PAz = p->d_prim + 7 * npp;
     t.cc = p->d_prim + 8 * npp;
 }
 
-static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vector<HostPair> &hp, cudaStream_t st)
+static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vector<HostPair> &hp, double thr, cudaStream_t st)
 {
     const adft_basis *b = p->basis;
     const size_t np = hp.size();
     std::vector<double> AB(3 * np);
-    std::vector<int32_t> pint(4 * np);
+    std::vector<int32_t> pint(5 * np);
     for (size_t g = 0; g < np; ++g) {
         const int sa = hp[g].sa, sb = hp[g].sb;
         for (int i = 0; i < 3; ++i) AB[i * np + g] = b->xyz[3 * b->atom[sa] + i] - b->xyz[3 * b->atom[sb] + i];
         pint[g] = b->bf_off[sa]; pint[np + g] = b->bf_off[sb]; pint[2 * np + g] = sa; pint[3 * np + g] = sb;
+        pint[4 * np + g] = hp[g].knom;
     }
     CUDA_TRY(cudaMemcpyAsync(p->d_AB, AB.data(), AB.size() * sizeof(double), cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(p->d_pint, pint.data(), pint.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
@@ -394,7 +434,8 @@ static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vecto
     double *f = p->d_prim;
     for (const Sublist &s : p->subl) {
         if (s.n == 0) continue;
-        pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, p->tab.sha, p->tab.shb, p->d_atom,
+        pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.la, s.lb, thr, nullptr,
+                                                             p->tab.sha, p->tab.shb, p->d_atom,
                                                              p->d_nprim, p->d_off, p->d_xyz, p->d_expo, p->d_coef, f, f + npp,
                                                              f + 2 * npp, f + 3 * npp, f + 4 * npp, f + 5 * npp, f + 6 * npp,
                                                              f + 7 * npp, f + 8 * npp);
@@ -403,9 +444,46 @@ static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vecto
     return ADFT_OK;
 }
 
+// Group (key, pair) records into sublists (same pair class and contraction depth): fills p->subl, p->subl_of_class,
+// hp (pairs in sublist order) and returns the number of primitive-pair records.
+struct BucketKey { int pc, K; bool operator<(const BucketKey &o) const { return pc != o.pc ? pc < o.pc : K < o.K; } };
+static int64_t make_sublists(adft_shellpairs *p, std::vector<std::pair<BucketKey, HostPair>> &all, std::vector<HostPair> &hp)
+{
+    const adft_basis *b = p->basis;
+    std::stable_sort(all.begin(), all.end(), [](const auto &x, const auto &y) { return x.first < y.first; });
+    hp.resize(all.size());
+    p->subl.clear();
+    for (auto &v : p->subl_of_class) v.clear();
+    int64_t prim_total = 0;
+    for (size_t g = 0; g < all.size();) {
+        size_t e = g;
+        while (e < all.size() && !(all[g].first < all[e].first)) ++e;
+        Sublist s;
+        s.pc = all[g].first.pc; s.K = all[g].first.K; s.n = (int)(e - g);
+        s.la = b->l[all[g].second.sa]; s.lb = b->l[all[g].second.sb];
+        s.pair_base = (int)g; s.prim_base = (int)prim_total;
+        prim_total += (int64_t)s.K * s.n;
+        p->subl_of_class[s.pc].push_back((int)p->subl.size());
+        p->subl.push_back(s);
+        for (size_t q = g; q < e; ++q) hp[q] = all[q].second;
+        g = e;
+    }
+    return prim_total;
+}
+
 extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda_stream, adft_shellpairs_t **out)
 {
+    return adft_shellpairs_build_ex(b, ADFT_DEFAULT_PRIM_THRESHOLD, cuda_stream, out);
+}
+
+extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double prim_threshold, void *cuda_stream,
+                                                  adft_shellpairs_t **out)
+{
     if (!b || !out) { set_error("adft_shellpairs_build: NULL"); return ADFT_ERR_INVALID_ARG; }
+    if (!(prim_threshold >= 0.0) || !std::isfinite(prim_threshold)) {
+        set_error("adft_shellpairs_build_ex: prim_threshold must be finite and >= 0");
+        return ADFT_ERR_INVALID_ARG;
+    }
     ensure_registered();
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
@@ -418,9 +496,9 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
     p->basis = b;
     const int ns = b->nshells;
 
+    p->prim_threshold = prim_threshold;
     // bucket pairs (A >= B) by pair class and contraction depth; a = the higher-l shell
-    struct Key { int pc, K; bool operator<(const Key &o) const { return pc != o.pc ? pc < o.pc : K < o.K; } };
-    std::vector<std::pair<Key, HostPair>> all;
+    std::vector<std::pair<BucketKey, HostPair>> all;
     all.reserve((size_t)ns * (ns + 1) / 2);
     for (int A = 0; A < ns; ++A)
         for (int B = 0; B <= A; ++B) {
@@ -439,27 +517,14 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
                 };
                 if (min_exp(sb) > min_exp(sa)) std::swap(sa, sb);
             }
-            all.push_back({Key{pair_class(b->l[sa], b->l[sb]), b->nprimv[sa] * b->nprimv[sb]}, HostPair{sa, sb, 0.0}});
+            const int knom = b->nprimv[sa] * b->nprimv[sb];
+            all.push_back({BucketKey{pair_class(b->l[sa], b->l[sb]), knom}, HostPair{sa, sb, 0.0, knom}});
         }
-    std::stable_sort(all.begin(), all.end(), [](const auto &x, const auto &y) { return x.first < y.first; });
-    std::vector<HostPair> hp(all.size());
+    std::vector<HostPair> hp;
     p->npairs = (int64_t)all.size();
-    int64_t prim_total = 0;
-    for (size_t g = 0; g < all.size();) {
-        size_t e = g;
-        while (e < all.size() && !(all[g].first < all[e].first)) ++e;
-        Sublist s;
-        s.pc = all[g].first.pc; s.K = all[g].first.K; s.n = (int)(e - g);
-        s.la = b->l[all[g].second.sa]; s.lb = b->l[all[g].second.sb];
-        s.pair_base = (int)g; s.prim_base = (int)prim_total;
-        prim_total += (int64_t)s.K * s.n;
-        p->subl_of_class[s.pc].push_back((int)p->subl.size());
-        p->subl.push_back(s);
-        for (size_t q = g; q < e; ++q) hp[q] = all[q].second;
-        g = e;
-    }
+    const int64_t prim_total = make_sublists(p, all, hp);
     if (prim_total > 0x7fffffffLL) { set_error("adft_shellpairs_build: too many primitive pairs"); free_pairs(p); return ADFT_ERR_ALLOC; }
-    p->nprimpairs = prim_total;
+    p->nprimpairs = p->nprimpairs_nominal = prim_total;
     // every needed Schwarz class must exist
     for (const Sublist &s : p->subl) {
         const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
@@ -483,10 +548,10 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
     ALLOC(p->d_off, ns * sizeof(int32_t));
     ALLOC(p->d_Q, np * sizeof(double));
     ALLOC(p->d_AB, 3 * np * sizeof(double));
-    ALLOC(p->d_pint, 4 * np * sizeof(int32_t));
+    ALLOC(p->d_pint, 5 * np * sizeof(int32_t));
     ALLOC(p->d_prim, 9 * npp * sizeof(double));
     ALLOC(p->d_boys, (size_t)BOYS_NT * BOYS_NM * sizeof(double));
-    ALLOC(p->d_counters, 3 * NQCLASS * sizeof(unsigned long long));
+    ALLOC(p->d_counters, 4 * NQCLASS * sizeof(unsigned long long));
     {
         // interpreter resources, only if some class that can occur lacks straight-line code
         int slots = 0;
@@ -541,8 +606,8 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
     TRY2(cudaMemcpyAsync(p->d_boys, boys.data(), boys.size() * sizeof(double), cudaMemcpyHostToDevice, st));
     TRY2(cudaStreamSynchronize(st));
 
-    // pass 1: records in bucket order, Schwarz bounds
-    rc = upload_pairs_and_prims(p, hp, st);
+    // pass 1: records of ALL primitive pairs in bucket order, Schwarz bounds from the full contraction
+    rc = upload_pairs_and_prims(p, hp, 0.0, st);
     if (rc) return fail(rc);
     for (const Sublist &s : p->subl) {
         if (s.n == 0) continue;
@@ -567,7 +632,34 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
         if (!std::isfinite(Q[g])) { set_error("adft_shellpairs_build: non-finite Schwarz bound"); return fail(ADFT_ERR_INTERNAL); }
         hp[g].Q = Q[g];
     }
-    // pass 2: sort every sublist by Q descending (ties: by shell indices, for determinism) and rebuild the records
+    // primitive screening (DESIGN R-11): number of primitive pairs of every pair whose estimate reaches the threshold
+    {
+        int32_t *d_kcount = p->d_pint + 4 * np;          // the knom slot is rewritten in pass 2
+        for (const Sublist &s : p->subl) {
+            if (s.n == 0) continue;
+            pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.la, s.lb, prim_threshold,
+                                                                 d_kcount, p->tab.sha, p->tab.shb, p->d_atom, p->d_nprim,
+                                                                 p->d_off, p->d_xyz, p->d_expo, p->d_coef, nullptr, nullptr,
+                                                                 nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+        }
+        TRY2(cudaGetLastError());
+        std::vector<int32_t> kc(np);
+        TRY2(cudaMemcpyAsync(kc.data(), d_kcount, np * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        TRY2(cudaStreamSynchronize(st));
+        // pass 2: re-bucket by (pair class, surviving depth), sort every sublist by Q descending (ties: by shell
+        // indices, for determinism) and rebuild the records
+        for (size_t g = 0; g < np; ++g) {
+            if (kc[g] < 1 || kc[g] > hp[g].knom) { set_error("adft_shellpairs_build: bad primitive count"); return fail(ADFT_ERR_INTERNAL); }
+            all[g] = {BucketKey{pair_class(b->l[hp[g].sa], b->l[hp[g].sb]), kc[g]}, hp[g]};
+        }
+        p->nprimpairs = make_sublists(p, all, hp);
+        if (p->nprimpairs < p->nprimpairs_nominal) {      // compact table: release the records of the dropped primitives
+            TRY2(cudaFree(p->d_prim));
+            p->d_prim = nullptr;
+            TRY2(cudaMalloc((void **)&p->d_prim, 9 * (size_t)p->nprimpairs * sizeof(double)));
+        }
+        set_table_pointers(p);
+    }
     for (const Sublist &s : p->subl)
         std::sort(hp.begin() + s.pair_base, hp.begin() + s.pair_base + s.n, [](const HostPair &x, const HostPair &y) {
             if (x.Q != y.Q) return x.Q > y.Q;
@@ -581,7 +673,7 @@ extern "C" adft_status_t adft_shellpairs_build(const adft_basis_t *b, void *cuda
         p->Qmat[(size_t)hp[g].sa * ns + hp[g].sb] = p->Qmat[(size_t)hp[g].sb * ns + hp[g].sa] = hp[g].Q;
     }
     TRY2(cudaMemcpyAsync(p->d_Q, p->hQ.data(), np * sizeof(double), cudaMemcpyHostToDevice, st));
-    rc = upload_pairs_and_prims(p, hp, st);
+    rc = upload_pairs_and_prims(p, hp, prim_threshold, st);
     if (rc) return fail(rc);
     TRY2(cudaStreamSynchronize(st));
 #undef TRY2
@@ -600,6 +692,14 @@ extern "C" adft_status_t adft_shellpairs_counts(const adft_shellpairs_t *p, int6
     if (!p) { set_error("adft_shellpairs_counts: NULL"); return ADFT_ERR_INVALID_ARG; }
     if (npairs) *npairs = p->npairs;
     if (nprimpairs) *nprimpairs = p->nprimpairs;
+    return ADFT_OK;
+}
+extern "C" adft_status_t adft_shellpairs_prim_counts(const adft_shellpairs_t *p, int64_t *nominal, int64_t *kept, double *threshold)
+{
+    if (!p) { set_error("adft_shellpairs_prim_counts: NULL"); return ADFT_ERR_INVALID_ARG; }
+    if (nominal) *nominal = p->nprimpairs_nominal;
+    if (kept) *kept = p->nprimpairs;
+    if (threshold) *threshold = p->prim_threshold;
     return ADFT_OK;
 }
 
@@ -707,7 +807,7 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         }
         if (o) CUDA_TRY(cudaMemcpyAsync(p->d_segs, p->h_segs, o * sizeof(Segment), cudaMemcpyHostToDevice, st));
     }
-    CUDA_TRY(cudaMemsetAsync(p->d_counters, 0, 3 * NQCLASS * sizeof(unsigned long long), st));
+    CUDA_TRY(cudaMemsetAsync(p->d_counters, 0, 4 * NQCLASS * sizeof(unsigned long long), st));
     if (J) CUDA_TRY(cudaMemsetAsync(J, 0, n2 * sizeof(double), st));
     if (K) CUDA_TRY(cudaMemsetAsync(K, 0, n2 * sizeof(double), st));
     CUDA_TRY(cudaEventRecord(ev_plan, st));
@@ -723,14 +823,14 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         JKParams prm{};
         prm.t = p->tab; prm.segs = p->d_segs + seg_off[qc]; prm.nsegs = (int)plan[qc].size(); prm.total_warps = warps[qc];
         prm.D = D; prm.J = Jw; prm.K = Kw; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boys;
-        prm.counters = p->d_counters + 2 * qc; prm.zero = 0;
+        prm.counters = p->d_counters + 4 * qc; prm.zero = 0;
         CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
         const ClassEntry &ce = class_table()[qc];
         if (ce.use_table) {
             InterpParams ip{};
             ip.jk = prm; ip.prog = make_prog(ce, p->d_blob, false);
             ip.scratch = p->d_scratch; ip.stride = p->scratch_threads;
-            ip.tile_counter = p->d_counters + 2 * NQCLASS + qc;
+            ip.tile_counter = p->d_counters + 4 * qc + 3;
             const long long want = (warps[qc] + 3) / 4;
             jk_interp_kernel<<<(unsigned)std::min<long long>(want, p->interp_blocks), 128, 0, st>>>(ip);
         } else {
@@ -762,16 +862,18 @@ extern "C" adft_status_t adft_jk_stats(adft_shellpairs_t *p, adft_jk_stats_t *ou
     if (!p || !out) { set_error("adft_jk_stats: NULL"); return ADFT_ERR_INVALID_ARG; }
     if (!p->have_build) { set_error("adft_jk_stats: no build yet"); return ADFT_ERR_INVALID_ARG; }
     cudaStream_t st = p->last_stream;
-    CUDA_TRY(cudaMemcpyAsync(p->h_small, p->d_counters, 2 * NQCLASS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(p->h_small, p->d_counters, 4 * NQCLASS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     adft_jk_stats_t &s = p->stats;
     cudaEvent_t *ev = p->ev;
-    s.quartets_kept = 0; s.prim_quartets = 0; s.model_flops = 0.0;
+    s.quartets_kept = 0; s.prim_quartets = 0; s.prim_quartets_evaluated = 0; s.model_flops = 0.0;
     for (int qc = 0; qc < NQCLASS; ++qc) {
-        s.class_quartets[qc] = (int64_t)p->h_small[2 * qc];
-        const int64_t prim = (int64_t)p->h_small[2 * qc + 1];
+        s.class_quartets[qc] = (int64_t)p->h_small[4 * qc];
+        const int64_t prim = (int64_t)p->h_small[4 * qc + 1];       // evaluated (after primitive screening)
         s.quartets_kept += s.class_quartets[qc];
-        s.prim_quartets += prim;
+        s.prim_quartets_evaluated += prim;
+        s.class_prim_quartets[qc] = prim;
+        s.prim_quartets += (int64_t)p->h_small[4 * qc + 2];
         const ClassEntry &ce = class_table()[qc];
         const int L = ce.la + ce.lb + ce.lc + ce.ld;
         // model flops: per primitive quartet 60+4L (geometry, prefactor, Boys) + generated VRR instructions

@@ -50,6 +50,7 @@ def check_full(api, orc, w, tau=None):
     assert st.quartets_unique == cnt["unique"]
     assert st.quartets_kept == cnt["kept"], (st.quartets_kept, cnt["kept"])
     assert st.prim_quartets == cnt["prim"]
+    assert 0 < st.prim_quartets_evaluated <= st.prim_quartets
     np.testing.assert_array_equal(np.array(st.class_quartets[:]), cnt["per_class"])
     assert np.abs(J - Jo).max() <= TOL_ELEM, np.abs(J - Jo).max()
     assert np.abs(K - Ko).max() <= TOL_ELEM, np.abs(K - Ko).max()
@@ -140,6 +141,35 @@ def test_j_only_k_only_and_repeat(api, orc):
         spread = max(spread, (J3 - J).abs().max().item(), (K3 - K).abs().max().item())
     assert spread <= 1e-11        # run-to-run spread from atomic ordering
     sp.close(); bs.close()
+
+
+def test_primitive_screening(api, orc):
+    """DESIGN R-11: the default primitive-pair threshold drops work but not accuracy; threshold 0 evaluates every
+    primitive quartet of the definition (what the oracle does); the Schwarz table never depends on the threshold."""
+    w = W.make(1)
+    bs = orc.basis_from_workload(w)
+    Jo, Ko, cnt = orc.jk(bs, w.D, w.tau)
+    J0, K0, st0, Q0 = api.jk(w, prim_threshold=0.0)
+    J1, K1, st1, Q1 = api.jk(w)
+    J2, K2, st2, Q2 = api.jk(w, prim_threshold=1e-9)          # far too coarse: must visibly change the result
+    assert np.array_equal(Q0, Q1) and np.array_equal(Q0, Q2)
+    assert st0.prim_quartets_evaluated == st0.prim_quartets == cnt["prim"]
+    assert st1.prim_quartets == cnt["prim"] and st1.prim_quartets_evaluated < st0.prim_quartets_evaluated
+    assert st2.prim_quartets_evaluated < st1.prim_quartets_evaluated
+    for st in (st0, st1, st2):
+        assert st.quartets_kept == cnt["kept"]
+    assert np.abs(J0 - Jo).max() <= TOL_ELEM and np.abs(K0 - Ko).max() <= TOL_ELEM
+    assert np.abs(J1 - J0).max() <= 1e-12 and np.abs(K1 - K0).max() <= 1e-12
+    assert np.abs(J2 - J0).max() > 1e-10
+    b = api.Basis.from_workload(w)
+    for bad in (-1.0, float("nan"), float("inf")):
+        with pytest.raises(api.AdftError) as e:
+            api.ShellPairs(b, prim_threshold=bad)
+        assert e.value.status == 1
+    sp = api.ShellPairs(b)
+    nominal, kept, thr = sp.prim_counts()
+    assert kept < nominal and thr == 1e-20
+    sp.close(); b.close()
 
 
 def test_error_codes_on_device(api):
