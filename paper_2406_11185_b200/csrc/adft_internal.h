@@ -27,7 +27,16 @@ struct ClassEntry {
     const int32_t *prog = nullptr;            // host copy of the class's table program (generated/programs.bin), if any
     int64_t prog_off = 0;                     // its offset in the blob (int32 units)
     bool use_table = false;                   // this class runs through the interpreter kernels (adft_interp.cuh)
+    bool use_rys = false;                     // this class runs through the block-cooperative Rys kernels (adft_rys.cuh)
 };
+
+// Rys kernels (adft_rys.cu): launchers per class, nullptr where none is instantiated
+struct RysTable;
+typedef cudaError_t (*rys_jk_fn)(const JKParams &p, const RysTable &rt, unsigned long long *tile_counter, cudaStream_t st);
+typedef cudaError_t (*rys_sw_fn)(const PairTable &t, const RysTable &rt, int pair_base, int prim_base, int n, int K,
+                                 double *Qout, cudaStream_t st);
+rys_jk_fn rys_jk_launcher(int la, int lb, int lc, int ld);
+rys_sw_fn rys_schwarz_launcher(int la, int lb);
 ClassEntry *class_table();                    // [NQCLASS]
 void register_all_classes();                  // defined in generated registry.cu
 

@@ -9,6 +9,7 @@
 
 #include "adft_internal.h"
 #include "adft_interp.cuh"
+#include "adft_rys.cuh"
 
 namespace adft {
 
@@ -23,6 +24,9 @@ static bool g_registered = false;
 // table programs of every class (generated/programs.bin, linked in through generated/programs_blob.S)
 extern "C" const int32_t adft_prog_blob[];
 extern "C" const int32_t adft_prog_blob_end[];
+// Rys root/weight tables (generated/rys_tables.bin from csrc/gen/gen_rys.py, linked in through generated/rys_blob.S)
+extern "C" const double adft_rys_blob[];
+extern "C" const double adft_rys_blob_end[];
 namespace adft {
 
 // program header fields (gen_eri.py pack_program)
@@ -46,9 +50,13 @@ static void ensure_registered()
         ClassEntry &e = g_classes[qc];
         e.prog = pr;
         e.prog_off = off;
+        const char *norys = getenv("ADFT_NO_RYS");
+        const bool have_rys = rys_jk_launcher(pr[PH_LA], pr[PH_LB], pr[PH_LC], pr[PH_LD]) != nullptr &&
+                              !(norys && norys[0] == '1');
         if (!e.launch_jk || force_table) {
-            e.use_table = true;
-            e.impl = "table";
+            e.use_rys = have_rys && !force_table;
+            e.use_table = !e.use_rys;
+            e.impl = e.use_rys ? "rys" : "table";
             e.la = pr[PH_LA]; e.lb = pr[PH_LB]; e.lc = pr[PH_LC]; e.ld = pr[PH_LD];
             e.vrr_ops = pr[PH_VRR_OPS]; e.hrr_ops = pr[PH_HRR_OPS]; e.nint = pr[PH_NINT];
         }
@@ -255,6 +263,8 @@ struct adft_shellpairs {
     size_t stage_n = 0;
     // interpreter path (classes without straight-line code): device copy of the program blob, per-thread scratch
     int32_t *d_blob = nullptr;
+    double *d_rys = nullptr;                  // device copy of the Rys tables
+    RysTable rys{};
     double *d_scratch = nullptr;
     long long scratch_threads = 0;     // threads of the persistent interpreter grid = scratch stride
     int interp_blocks = 0;
@@ -392,7 +402,7 @@ static void free_pairs(adft_shellpairs *p)
     cudaFree(p->d_xyz); cudaFree(p->d_expo); cudaFree(p->d_coef); cudaFree(p->d_atom); cudaFree(p->d_nprim);
     cudaFree(p->d_off); cudaFree(p->d_Q); cudaFree(p->d_AB); cudaFree(p->d_prim); cudaFree(p->d_pint);
     cudaFree(p->d_boys); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage); cudaFree(p->d_sink);
-    cudaFree(p->d_blob); cudaFree(p->d_scratch);
+    cudaFree(p->d_blob); cudaFree(p->d_scratch); cudaFree(p->d_rys);
     if (p->h_segs) cudaFreeHost(p->h_segs);
     if (p->h_small) cudaFreeHost(p->h_small);
     if (p->ev_ok) for (auto &e : p->ev) cudaEventDestroy(e);
@@ -560,7 +570,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
                 if (p->subl_of_class[X].empty() || p->subl_of_class[Y].empty()) continue;
                 const ClassEntry &ce = class_table()[quartet_class(X, Y)];
                 if (ce.use_table) slots = std::max(slots, jk_slots_of(ce));
-                if (X == Y && (ce.use_table || !ce.launch_schwarz)) slots = std::max(slots, schwarz_slots_of(ce));
+                if (X == Y && (ce.use_table || (!ce.launch_schwarz && !ce.use_rys))) slots = std::max(slots, schwarz_slots_of(ce));
             }
         if (slots > 0) {
             int dev = 0, sms = 0;
@@ -573,7 +583,20 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
         }
     }
     ALLOC(p->d_dmax, 2 * sizeof(unsigned long long));
+    ALLOC(p->d_rys, (size_t)(adft_rys_blob_end - adft_rys_blob) * sizeof(double));
 #undef ALLOC
+    {
+        // Rys tables (gen_rys.py layout): header[8] = magic, NMAX, TMAX, H, NCOEF
+        const double *h = adft_rys_blob;
+        const int nmax = (int)h[1], ncoef = (int)h[4];
+        const int nint = (int)std::lround(h[2] / h[3]);
+        if (h[0] != 5259531.0 || nmax < 7) { set_error("adft_shellpairs_build: bad Rys table blob"); free_pairs(p); return ADFT_ERR_INTERNAL; }
+        p->rys.tab = p->d_rys; p->rys.nint = nint; p->rys.ncoef = ncoef; p->rys.tmax = h[2]; p->rys.inv_h = 1.0 / h[3];
+        int off = 8;
+        for (int n = 1; n <= 7; ++n) { p->rys.off_cheb[n] = off; off += nint * 2 * n * ncoef; }
+        for (int n = 1; n <= 7; ++n) { p->rys.off_asym[n] = off; off += 2 * n; }
+        if (off != (int)(adft_rys_blob_end - adft_rys_blob)) { set_error("adft_shellpairs_build: Rys table size mismatch"); free_pairs(p); return ADFT_ERR_INTERNAL; }
+    }
     if (cudaMallocHost((void **)&p->h_small, 4 * NQCLASS * sizeof(unsigned long long)) != cudaSuccess) {
         set_error("adft_shellpairs_build: cudaMallocHost failed"); free_pairs(p); return ADFT_ERR_ALLOC;
     }
@@ -598,6 +621,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     TRY2(cudaMemcpyAsync(p->d_atom, b->atom.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     TRY2(cudaMemcpyAsync(p->d_nprim, b->nprimv.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     TRY2(cudaMemcpyAsync(p->d_off, b->off.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    TRY2(cudaMemcpyAsync(p->d_rys, adft_rys_blob, (size_t)(adft_rys_blob_end - adft_rys_blob) * sizeof(double),
+                         cudaMemcpyHostToDevice, st));
     if (p->d_blob)
         TRY2(cudaMemcpyAsync(p->d_blob, adft_prog_blob, (size_t)(adft_prog_blob_end - adft_prog_blob) * sizeof(int32_t),
                              cudaMemcpyHostToDevice, st));
@@ -614,6 +639,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
         const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
         if (ce.launch_schwarz && !ce.use_table) {
             ce.launch_schwarz(p->tab, s.pair_base, s.prim_base, s.n, s.K, p->d_boys, p->d_Q, st);
+        } else if (ce.use_rys && rys_schwarz_launcher(s.la, s.lb)) {
+            TRY2(rys_schwarz_launcher(s.la, s.lb)(p->tab, p->rys, s.pair_base, s.prim_base, s.n, s.K, p->d_Q, st));
         } else {
             const InterpProg pg = make_prog(ce, p->d_blob, true);
             for (long long first = 0; first < s.n; first += p->scratch_threads) {
@@ -759,7 +786,7 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
     for (int X = 0; X < NPAIRCLASS; ++X)
         for (int Y = 0; Y <= X; ++Y)
             if (!p->subl_of_class[X].empty() && !p->subl_of_class[Y].empty() && !class_table()[quartet_class(X, Y)].launch_jk &&
-                !class_table()[quartet_class(X, Y)].use_table) {
+                !class_table()[quartet_class(X, Y)].use_table && !class_table()[quartet_class(X, Y)].use_rys) {
                 set_error("adft_jk_build: no kernel compiled for quartet class " + std::to_string(quartet_class(X, Y)));
                 return ADFT_ERR_UNSUPPORTED_L;
             }
@@ -826,7 +853,9 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         prm.counters = p->d_counters + 4 * qc; prm.zero = 0;
         CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
         const ClassEntry &ce = class_table()[qc];
-        if (ce.use_table) {
+        if (ce.use_rys) {
+            CUDA_TRY(rys_jk_launcher(ce.la, ce.lb, ce.lc, ce.ld)(prm, p->rys, p->d_counters + 4 * qc + 3, st));
+        } else if (ce.use_table) {
             InterpParams ip{};
             ip.jk = prm; ip.prog = make_prog(ce, p->d_blob, false);
             ip.scratch = p->d_scratch; ip.stride = p->scratch_threads;

@@ -431,6 +431,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", required=True)
     ap.add_argument("--max-nacc", type=int, default=1000, help="largest NE*NF emitted as straight-line code")
+    ap.add_argument("--max-l2-nacc", type=int, default=1000, help="the same limit for classes without f shells")
     ap.add_argument("--max-l", type=int, default=2, help="highest shell l emitted as straight-line code")
     ap.add_argument("--cmax", type=str, default="{}", help="JSON {tag: [chunk sizes]} of multi-pass variants to emit")
     args = ap.parse_args()
@@ -440,7 +441,7 @@ def main():
     for (la, lb, lc, ld) in all_classes(3):
         NE = sum(ncart(e) for e in range(la, la + lb + 1))
         NF = sum(ncart(f) for f in range(lc, lc + ld + 1))
-        if max(la, lb, lc, ld) > args.max_l or NE * NF > args.max_nacc:
+        if max(la, lb, lc, ld) > args.max_l or NE * NF > (args.max_nacc if la == 3 else args.max_l2_nacc):
             continue
         src, meta = generate_class(la, lb, lc, ld, cmax_map.get(class_tag(la, lb, lc, ld), ()))
         with open(os.path.join(args.out, f"eri_{meta['tag']}.cuh"), "w") as f:
