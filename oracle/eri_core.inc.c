@@ -131,6 +131,7 @@ typedef struct {
     REAL *hb;    /* bra HRR   [NCUM_B][NCUM_MAX][NCUM_MAX] */
     REAL *g;     /* (ab|c0)   [nA*nB][NCUM_MAX] */
     REAL *hk;    /* ket HRR   [NCUM_B][NCUM_MAX] */
+    REAL *part;  /* one orientation's contribution  [NCART_MAX^4] */
 } NAME(scratch_t);
 
 static int NAME(scratch_alloc)(NAME(scratch_t) *s)
@@ -140,18 +141,24 @@ static int NAME(scratch_alloc)(NAME(scratch_t) *s)
     s->hb = (REAL *)malloc(sizeof(REAL) * (size_t)NCUM_B * NCUM_MAX * NCUM_MAX);
     s->g = (REAL *)malloc(sizeof(REAL) * (size_t)NCART_MAX * NCART_MAX * NCUM_MAX);
     s->hk = (REAL *)malloc(sizeof(REAL) * (size_t)NCUM_B * NCUM_MAX);
-    return (s->v && s->acc && s->hb && s->g && s->hk) ? 0 : -1;
+    s->part = (REAL *)malloc(sizeof(REAL) * (size_t)NCART_MAX * NCART_MAX * NCART_MAX * NCART_MAX);
+    return (s->v && s->acc && s->hb && s->g && s->hk && s->part) ? 0 : -1;
 }
 static void NAME(scratch_free)(NAME(scratch_t) *s)
 {
-    free(s->v); free(s->acc); free(s->hb); free(s->g); free(s->hk);
+    free(s->v); free(s->acc); free(s->hb); free(s->g); free(s->hk); free(s->part);
 }
 
-/* All nA*nB*nC*nD contracted integrals of one shell quartet, out[((ia*nB+ib)*nC+ic)*nD+id].
- * Coefficients ca..cd are FINAL contraction coefficients d_k (SURVEY R-1). */
-static void NAME(shell_quartet)(const basis_t *bs, int sA, int sB, int sC, int sD,
-                                NAME(scratch_t) *s, REAL *out)
+/* Contribution to the nA*nB*nC*nD contracted integrals of one shell quartet, out[((ia*nB+ib)*nC+ic)*nD+id], of the
+ * primitive quartets selected by (tieAB, tieCD): the recurrences are built on sA and sC (VRR) and shifted onto sB and
+ * sD (HRR), and a primitive pair (alpha on sA, beta on sB) takes part iff the Gaussian product centre
+ * P = (alpha A + beta B)/(alpha+beta) is nearer to sA than to sB, i.e. alpha > beta, or alpha == beta when tieAB != 0;
+ * likewise for (sC, sD) with tieCD  (reading R-22).  Returns the number of primitive quartets it summed.
+ * Coefficients are FINAL contraction coefficients d_k (SURVEY R-1). */
+static long NAME(shell_quartet_part)(const basis_t *bs, int sA, int sB, int sC, int sD, int tieAB, int tieCD,
+                                     NAME(scratch_t) *s, REAL *out)
 {
+    long nsummed = 0;
     const int la = bs->l[sA], lb = bs->l[sB], lc = bs->l[sC], ld = bs->l[sD];
     const int lab = la + lb, lcd = lc + ld;
     REAL A[3], B[3], C[3], D[3];
@@ -169,11 +176,15 @@ static void NAME(shell_quartet)(const basis_t *bs, int sA, int sB, int sC, int s
     for (int ic = 0; ic < bs->nprim[sC]; ++ic)
     for (int id = 0; id < bs->nprim[sD]; ++id) {
         int oa = bs->off[sA] + ia, ob = bs->off[sB] + ib, oc = bs->off[sC] + ic, od = bs->off[sD] + id;
+        if (!(bs->expo[oa] > bs->expo[ob] || (tieAB && bs->expo[oa] == bs->expo[ob]))) continue;
+        if (!(bs->expo[oc] > bs->expo[od] || (tieCD && bs->expo[oc] == bs->expo[od]))) continue;
+        ++nsummed;
         REAL coef = (REAL)bs->coef[oa] * (REAL)bs->coef[ob] * (REAL)bs->coef[oc] * (REAL)bs->coef[od];
         NAME(prim_vrr)(lab, lcd, bs->expo[oa], bs->expo[ob], bs->expo[oc], bs->expo[od], A, B, C, D, coef, v);
         for (int a = NCUM(la - 1); a < NCUM(lab); ++a)
             for (int c = NCUM(lc - 1); c < NCUM(lcd); ++c) acc[a * NCUM_MAX + c] += V(0, a, c);
     }
+    if (nsummed == 0) return 0;
 
     /* HRR on the bra: (a, b+1_i| c) = (a+1_i, b| c) + (A_i - B_i)(a b| c) */
 #define HB(b, a, c) s->hb[((size_t)(b) * NCUM_MAX + (a)) * NCUM_MAX + (c)]
@@ -223,5 +234,34 @@ static void NAME(shell_quartet)(const basis_t *bs, int sA, int sB, int sC, int s
     }
 #undef HB
 #undef HK
+    return nsummed;
+}
+
+/* All nA*nB*nC*nD contracted integrals of one shell quartet, out[((ia*nB+ib)*nC+ic)*nD+id]: the sum over primitive
+ * quartets is split into the four groups {P nearer A | P nearer B} x {Q nearer C | Q nearer D}; each group is evaluated
+ * with the recurrences built on the nearer centres (the bra or ket pair handed over in swapped order, which is the
+ * identity (ab|cd) = (ba|cd) = (ab|dc) of the definition) and the four results are added.
+ * Why: the horizontal recurrence (a,b+1_i| = (a+1_i,b| + (A_i-B_i)(ab| subtracts numbers of size |A-B|^lb when P sits
+ * on B; built on the nearer centre the shifted factor (x-B_i) = (x-P_i) + (P_i-B_i) stays small.  R-22. */
+static void NAME(shell_quartet)(const basis_t *bs, int sA, int sB, int sC, int sD,
+                                NAME(scratch_t) *s, REAL *out)
+{
+    const int nA = NCART(bs->l[sA]), nB = NCART(bs->l[sB]), nC = NCART(bs->l[sC]), nD = NCART(bs->l[sD]);
+    for (int q = 0; q < nA * nB * nC * nD; ++q) out[q] = 0;
+    for (int swab = 0; swab < 2; ++swab)
+    for (int swcd = 0; swcd < 2; ++swcd) {
+        REAL *part = s->part;
+        long n = NAME(shell_quartet_part)(bs, swab ? sB : sA, swab ? sA : sB, swcd ? sD : sC, swcd ? sC : sD,
+                                          !swab, !swcd, s, part);
+        if (n == 0) continue;
+        const int n2 = swab ? nA : nB, n3 = swcd ? nD : nC, n4 = swcd ? nC : nD;
+        for (int ia = 0; ia < nA; ++ia)
+        for (int ib = 0; ib < nB; ++ib)
+        for (int ic = 0; ic < nC; ++ic)
+        for (int id = 0; id < nD; ++id) {
+            const int i1 = swab ? ib : ia, i2 = swab ? ia : ib, i3 = swcd ? id : ic, i4 = swcd ? ic : id;
+            out[((ia * nB + ib) * nC + ic) * nD + id] += part[((i1 * n2 + i2) * n3 + i3) * n4 + i4];
+        }
+    }
 }
 #undef V

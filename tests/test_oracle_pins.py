@@ -339,3 +339,41 @@ def test_p13_documented_hrr_cancellation_case(orc):
     Q = orc.schwarz(bs)
     diag = max(float(abs(ld1[i, j, i, j])) for i in range(ld1.shape[0]) for j in range(ld1.shape[1]))
     assert Q[A, B] == pytest.approx(np.sqrt(diag), rel=1e-13)         # ... and the Schwarz table uses the ld core
+
+
+@pytest.mark.parametrize("ls", [(1, 3), (3, 3), (0, 3), (2, 3), (3, 1)])
+def test_p15_recurrence_centre_order_independence(orc, ls):
+    """DESIGN.md R-22: every primitive quartet is evaluated with the recurrences built on the centre nearest to its
+    Gaussian product centre, so the identity (ab|cd) = (ba|cd) = (ab|dc) = (ba|dc) of the definition
+    must hold to rounding whichever order the shells are handed over in -- also in plain fp64, also for the case that
+    broke the single-orientation core: a very tight high-l shell 11 bohr from a shell with a diffuse primitive
+    (cfg 3 shells (242, 294): relative error 33% on Q in long double before R-22).  A wrong index permutation when the
+    four orientation groups are added, or a primitive pair counted in two groups or in none, fails this test."""
+    atoms = np.array([[0.0, 0.0, 0.0], [6.3, -7.1, 5.4], [0.4, 1.1, -0.3], [5.9, -6.5, 5.0]])
+    la, lb = ls
+    exps = {0: [4595.251], 1: [38.639, 0.05, 376.079], 2: [2019.87, 0.246, 4.992], 3: [1.7, 0.3]}
+    cofs = {0: [0.75], 1: [1.0, 0.77, 0.34], 2: [0.53, 0.22, 0.17], 3: [0.6, 0.4]}
+    lsh = [lb, la, la, lb]            # shell 0 (tight, single primitive) carries lb; shell 1 (mixed) carries la
+    s_np = np.array([len(exps[i]) for i in range(4)], np.int32)
+    s_off = np.concatenate([[0], np.cumsum(s_np)[:-1]]).astype(np.int32)
+    e = np.array(sum((exps[i] for i in range(4)), []), np.float64)
+    c = np.array(sum((cofs[i] for i in range(4)), []), np.float64)
+    nbf = sum((l + 1) * (l + 2) // 2 for l in lsh)
+    w = W.Workload("p15", atoms, np.arange(4, dtype=np.int32), np.array(lsh, np.int32), s_np, s_off, e, c,
+                   np.eye(nbf), 0.0)
+    bs = orc.basis_from_workload(w)
+    for ld in (False, True):
+        ref = orc.eri_block(bs, 0, 1, 2, 3, long_double=ld).astype(np.float64)
+        scale = float(np.abs(ref).max())
+        assert scale > 0
+        for perm, tr in (((1, 0, 2, 3), (1, 0, 2, 3)), ((0, 1, 3, 2), (0, 1, 3, 2)), ((1, 0, 3, 2), (1, 0, 3, 2))):
+            sh = [0, 1, 2, 3]
+            other = orc.eri_block(bs, *[sh[p] for p in perm], long_double=ld).astype(np.float64).transpose(tr)
+            assert float(np.abs(other - ref).max()) <= 2e-13 * scale
+    # fp64 and long double agree: nothing left for extra precision to repair
+    d = orc.eri_block(bs, 0, 1, 2, 3); l_ = orc.eri_block(bs, 0, 1, 2, 3, long_double=True).astype(np.float64)
+    assert float(np.abs(d - l_).max()) <= 2e-13 * float(np.abs(l_).max())
+    # the pair that exposed it: diagonal block in both orders
+    for (A, B) in ((0, 1),):
+        b1 = orc.eri_block(bs, A, B, A, B); b2 = orc.eri_block(bs, B, A, B, A).transpose(1, 0, 3, 2)
+        assert float(np.abs(b1 - b2).max()) <= 2e-13 * float(np.abs(b1).max())
