@@ -146,24 +146,22 @@ __global__ void __launch_bounds__(128) jk_interp_kernel(const InterpParams q)
         }
         const Segment sg = p.segs[lo];
         const long long r = w - sg.warp_begin;
-        const int i = (int)(r / sg.tiles_per_row);
-        const int tile = (int)(r % sg.tiles_per_row);
+        int i = (int)(r / sg.tiles_per_row) * TILE_R + lane / TILE_C;
+        int j = (int)(r % sg.tiles_per_row) * TILE_C + (lane & (TILE_C - 1));
+        bool valid = i < sg.rows && j < (sg.same ? (i + 1) : sg.ket_n);
+        if (!valid) { i = 0; j = 0; }
         const int gab = sg.bra_pair_base + i;
         const double Qab = __ldg(p.t.Q + gab);
-        const int jlim = sg.same ? (i + 1) : sg.ket_n;
-        int j = tile * 32 + lane;
-        bool valid = j < jlim;
-        if (!valid) j = 0;
         const int gcd = sg.ket_pair_base + j;
         valid = valid && ((Qab * __ldg(p.t.Q + gcd)) * p.dmax >= p.tau);      // the screen (DESIGN R-7)
         const unsigned ballot = __ballot_sync(0xffffffffu, valid);
         if (ballot == 0u) continue;
-        const unsigned knom_cd = __reduce_add_sync(0xffffffffu, valid ? (unsigned)__ldg(p.t.knom + gcd) : 0u);
+        const unsigned knom = __reduce_add_sync(0xffffffffu, valid ? (unsigned)(__ldg(p.t.knom + gab) * __ldg(p.t.knom + gcd)) : 0u);
         if (lane == 0) {
             const unsigned long long n = (unsigned long long)__popc(ballot);
             cnt_q += n;
             cnt_p += n * (unsigned long long)(sg.bra_K * sg.ket_K);
-            cnt_n += (unsigned long long)__ldg(p.t.knom + gab) * knom_cd;
+            cnt_n += (unsigned long long)knom;
         }
         for (int x = 0; x < pg.nacc; ++x) A[x * st] = 0.0;
         for (int kb = 0; kb < sg.bra_K; ++kb) {
@@ -219,8 +217,8 @@ __global__ void __launch_bounds__(128) jk_interp_kernel(const InterpParams q)
         double *J = p.J, *K = p.K;
         for (int x = 0; x < na * nb; ++x) {
             double v = jab[x * st];
-            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-            if (lane == 0) atomicAdd(J + (size_t)(a0 + x / nb) * N + b0 + x % nb, v);
+            for (int o = TILE_C / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if ((lane & (TILE_C - 1)) == 0 && v != 0.0) atomicAdd(J + (size_t)(a0 + x / nb) * N + b0 + x % nb, v);
         }
         if (valid) {
             for (int x = 0; x < nc * nd; ++x) atomicAdd(J + (size_t)(c0 + x / nd) * N + d0 + x % nd, jcd[x * st]);

@@ -759,7 +759,7 @@ static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax,
             Segment sg{};
             sg.bra_pair_base = s1.pair_base; sg.bra_prim_base = s1.prim_base; sg.bra_n = s1.n; sg.bra_K = s1.K;
             sg.ket_pair_base = s2.pair_base; sg.ket_prim_base = s2.prim_base; sg.ket_n = s2.n; sg.ket_K = s2.K;
-            sg.rows = rows; sg.tiles_per_row = (cols + 31) / 32; sg.same = same ? 1 : 0;
+            sg.rows = rows; sg.tiles_per_row = (cols + TILE_C - 1) / TILE_C; sg.same = same ? 1 : 0;
             segs.push_back(sg);
         }
     // heaviest tiles first (per-tile cost ~ K1*K2), so the tail of the launch is made of cheap tiles
@@ -767,7 +767,7 @@ static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax,
         return (long long)a.bra_K * a.ket_K > (long long)b.bra_K * b.ket_K;
     });
     long long w = 0;
-    for (Segment &s : segs) { s.warp_begin = w; w += (long long)s.rows * s.tiles_per_row; }
+    for (Segment &s : segs) { s.warp_begin = w; w += (long long)((s.rows + TILE_R - 1) / TILE_R) * s.tiles_per_row; }
     return w;
 }
 

@@ -111,9 +111,14 @@ struct RysCfg {
 
 // phase 1: the 2-D integrals of one (primitive quartet, root, axis), all (i<=la, j<=lb, k<=lc, l<=ld), to `out`
 // (layout out[(i*(LB+1)+j)*PADCD + k*(LD+1)+l]).  The z axis carries prefactor * weight.
+// Recurrence centre (R-22): the vertical recurrence is built on whichever shell of the pair is nearer to
+// this primitive pair's product centre (B instead of A iff |P-B| < |P-A|, D instead of C iff |Q-D| < |Q-C|) and the
+// horizontal transfer runs towards the other shell, so the transferred factor (x - far centre) = (x - near centre) +
+// (near - far) never has to cancel a large recurrence value.  The choice costs nothing here because the transfer is
+// done per primitive in 2-D.
 template <class C>
 __device__ __forceinline__ void rys_phase1(const RysTable &rt, const PrimPair &b, const PrimPair &k, int r, int ax,
-                                           double AB, double CD, double *__restrict__ out)
+                                           const double (&ABv)[3], const double (&CDv)[3], double *__restrict__ out)
 {
     constexpr int NBR = C::LA + C::LB, NKT = C::LC + C::LD;
     const double s = b.zeta + k.zeta;
@@ -126,8 +131,14 @@ __device__ __forceinline__ void rys_phase1(const RysTable &rt, const PrimPair &b
     double u, w;
     rys_root<C::NR>(rt, T, r, u, w);
     const double pq = ax == 0 ? PQx : (ax == 1 ? PQy : PQz);
-    const double pa = ax == 0 ? b.PAx : (ax == 1 ? b.PAy : b.PAz);
-    const double qc = ax == 0 ? k.PAx : (ax == 1 ? k.PAy : k.PAz);
+    const double PBx = b.PAx + ABv[0], PBy = b.PAy + ABv[1], PBz = b.PAz + ABv[2];       // P - B
+    const double QDx = k.PAx + CDv[0], QDy = k.PAy + CDv[1], QDz = k.PAz + CDv[2];       // Q - D
+    const bool onB = fma(PBx, PBx, fma(PBy, PBy, PBz * PBz)) < fma(b.PAx, b.PAx, fma(b.PAy, b.PAy, b.PAz * b.PAz));
+    const bool onD = fma(QDx, QDx, fma(QDy, QDy, QDz * QDz)) < fma(k.PAx, k.PAx, fma(k.PAy, k.PAy, k.PAz * k.PAz));
+    const double AB = ax == 0 ? ABv[0] : (ax == 1 ? ABv[1] : ABv[2]);
+    const double CD = ax == 0 ? CDv[0] : (ax == 1 ? CDv[1] : CDv[2]);
+    const double pa = (ax == 0 ? b.PAx : (ax == 1 ? b.PAy : b.PAz)) + (onB ? AB : 0.0);   // P - (A or B)
+    const double qc = (ax == 0 ? k.PAx : (ax == 1 ? k.PAy : k.PAz)) + (onD ? CD : 0.0);   // Q - (C or D)
     const double B00 = 0.5 * u * inv_s;
     const double B10 = b.inv2z * fma(-roz, u, 1.0);
     const double B01 = k.inv2z * fma(-roe, u, 1.0);
@@ -151,20 +162,33 @@ __device__ __forceinline__ void rys_phase1(const RysTable &rt, const PrimPair &b
             g[n][m + 1] = v;
         }
     }
-    // ket transfer (k on C, l on D), then bra transfer (i on A, j on B)
+    // ket transfer (k on C, l on D), then bra transfer (i on A, j on B); from the near centre towards the far one:
+    //   built on C: (k, l+1) = (k+1, l) + (C-D)(k, l)        built on D: (k+1, l) = (k, l+1) + (D-C)(k, l)
     double kt[NBR + 1][C::NKL];
 #pragma unroll
     for (int n = 0; n <= NBR; ++n) {
         double h[NKT + 1];
 #pragma unroll
         for (int m = 0; m <= NKT; ++m) h[m] = g[n][m];
+        if (!onD) {
 #pragma unroll
-        for (int l = 0; l <= C::LD; ++l) {
+            for (int l = 0; l <= C::LD; ++l) {
 #pragma unroll
-            for (int kk = 0; kk <= C::LC; ++kk) kt[n][kk * (C::LD + 1) + l] = h[kk];
-            if (l < C::LD) {
+                for (int kk = 0; kk <= C::LC; ++kk) kt[n][kk * (C::LD + 1) + l] = h[kk];
+                if (l < C::LD) {
 #pragma unroll
-                for (int m = 0; m < NKT - l; ++m) h[m] = fma(CD, h[m], h[m + 1]);
+                    for (int m = 0; m < NKT - l; ++m) h[m] = fma(CD, h[m], h[m + 1]);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int kk = 0; kk <= C::LC; ++kk) {
+#pragma unroll
+                for (int l = 0; l <= C::LD; ++l) kt[n][kk * (C::LD + 1) + l] = h[l];
+                if (kk < C::LC) {
+#pragma unroll
+                    for (int m = 0; m < NKT - kk; ++m) h[m] = fma(-CD, h[m], h[m + 1]);
+                }
             }
         }
     }
@@ -173,13 +197,25 @@ __device__ __forceinline__ void rys_phase1(const RysTable &rt, const PrimPair &b
         double f[NBR + 1];
 #pragma unroll
         for (int n = 0; n <= NBR; ++n) f[n] = kt[n][kl];
+        if (!onB) {
 #pragma unroll
-        for (int j = 0; j <= C::LB; ++j) {
+            for (int j = 0; j <= C::LB; ++j) {
 #pragma unroll
-            for (int i = 0; i <= C::LA; ++i) out[(i * (C::LB + 1) + j) * C::PADCD + kl] = f[i];
-            if (j < C::LB) {
+                for (int i = 0; i <= C::LA; ++i) out[(i * (C::LB + 1) + j) * C::PADCD + kl] = f[i];
+                if (j < C::LB) {
 #pragma unroll
-                for (int n = 0; n < NBR - j; ++n) f[n] = fma(AB, f[n], f[n + 1]);
+                    for (int n = 0; n < NBR - j; ++n) f[n] = fma(AB, f[n], f[n + 1]);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i <= C::LA; ++i) {
+#pragma unroll
+                for (int j = 0; j <= C::LB; ++j) out[(i * (C::LB + 1) + j) * C::PADCD + kl] = f[j];
+                if (i < C::LA) {
+#pragma unroll
+                    for (int n = 0; n < NBR - i; ++n) f[n] = fma(-AB, f[n], f[n + 1]);
+                }
             }
         }
     }
@@ -337,8 +373,7 @@ __device__ __forceinline__ void rys_quartet(const PairTable &t, const RysTable &
             const int kb = pq / ket_K, kk = pq - kb * ket_K;
             const PrimPair bp = load_prim(t, bra_prim + kb * bra_stride);
             const PrimPair kp = load_prim(t, ket_prim + kk * ket_stride);
-            rys_phase1<C>(rt, bp, kp, r, ax, ax == 0 ? AB[0] : (ax == 1 ? AB[1] : AB[2]), ax == 0 ? CD[0] : (ax == 1 ? CD[1] : CD[2]),
-                          sm + it * C::ITEMSZ + ax * C::AXSZ);
+            rys_phase1<C>(rt, bp, kp, r, ax, AB, CD, sm + it * C::ITEMSZ + ax * C::AXSZ);
         }
         __syncthreads();
         rys_phase2_dispatch<C>(chunk, sm, nb, offx, offy, offz, acc);
@@ -372,25 +407,21 @@ __global__ void __launch_bounds__(C::NT, 1) jk_rys_kernel(const JKParams p, cons
         }
         const Segment sg = p.segs[lo];
         const long long r = w - sg.warp_begin;
-        const int i = (int)(r / sg.tiles_per_row);
-        const int tile = (int)(r % sg.tiles_per_row);
-        const int gab = sg.bra_pair_base + i;
-        const double Qab = __ldg(p.t.Q + gab);
-        const int jlim = sg.same ? (i + 1) : sg.ket_n;
-        const int sa = __ldg(p.t.sha + gab), sb = __ldg(p.t.shb + gab);
-        const int a0 = __ldg(p.t.bfa + gab), b0 = __ldg(p.t.bfb + gab);
-        const double AB[3] = {__ldg(p.t.ABx + gab), __ldg(p.t.ABy + gab), __ldg(p.t.ABz + gab)};
-        const unsigned knom_ab = (unsigned)__ldg(p.t.knom + gab);
-        for (int jj = 0; jj < 32; ++jj) {
-            const int j = tile * 32 + jj;
-            if (j >= jlim) break;
-            const int gcd = sg.ket_pair_base + j;
-            if (!((Qab * __ldg(p.t.Q + gcd)) * p.dmax >= p.tau)) continue;      // the screen (DESIGN R-7)
+        const int i_base = (int)(r / sg.tiles_per_row) * TILE_R, j_base = (int)(r % sg.tiles_per_row) * TILE_C;
+        for (int jj = 0; jj < 32; ++jj) {                       // the 32 quartets of the tile, one after the other
+            const int i = i_base + jj / TILE_C, j = j_base + (jj & (TILE_C - 1));
+            if (i >= sg.rows) break;
+            if (j >= (sg.same ? (i + 1) : sg.ket_n)) continue;
+            const int gab = sg.bra_pair_base + i, gcd = sg.ket_pair_base + j;
+            if (!((__ldg(p.t.Q + gab) * __ldg(p.t.Q + gcd)) * p.dmax >= p.tau)) continue;   // the screen (DESIGN R-7)
             if (tid == 0) {
                 cnt_q += 1ull;
                 cnt_p += (unsigned long long)(sg.bra_K * sg.ket_K);
-                cnt_n += (unsigned long long)knom_ab * (unsigned)__ldg(p.t.knom + gcd);
+                cnt_n += (unsigned long long)((unsigned)__ldg(p.t.knom + gab) * (unsigned)__ldg(p.t.knom + gcd));
             }
+            const int sa = __ldg(p.t.sha + gab), sb = __ldg(p.t.shb + gab);
+            const int a0 = __ldg(p.t.bfa + gab), b0 = __ldg(p.t.bfb + gab);
+            const double AB[3] = {__ldg(p.t.ABx + gab), __ldg(p.t.ABy + gab), __ldg(p.t.ABz + gab)};
             const double CD[3] = {__ldg(p.t.ABx + gcd), __ldg(p.t.ABy + gcd), __ldg(p.t.ABz + gcd)};
             double acc[C::CH];
             rys_quartet<C>(p.t, rt, sm, sg.bra_prim_base + i, sg.bra_n, sg.bra_K, sg.ket_prim_base + j, sg.ket_n, sg.ket_K,
