@@ -33,9 +33,21 @@ for X, (la, lb) in enumerate(PAIR_CLASSES):
     for Y, (lc, ld) in enumerate(PAIR_CLASSES[:X + 1]):
         CLASS_NAMES.append("(%s%s|%s%s)" % ("spdf"[la], "spdf"[lb], "spdf"[lc], "spdf"[ld]))
 
+# classes that run through the block-cooperative Rys kernels (csrc/adft_rys.cu); all others are generated straight-line code
+RYS_CLASSES = {"(fp|fp)", "(ff|pp)", "(fd|dp)", "(ff|fs)", "(fp|dd)", "(fd|fp)", "(ff|dp)", "(fd|dd)", "(ff|fp)", "(fd|fd)",
+               "(ff|dd)", "(ff|fd)", "(ff|ff)"}
 WORKLOAD_NAMES = {0: "cfg0_3atom_13bf", 1: "cfg1_10atom_chain_100bf", 2: "cfg2_60atom_cluster_500bf",
                   3: "cfg3_60atom_cluster_f_940bf", 4: "cfg4_300atom_globular_2500bf"}
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA/clk x 2 flops x 1.965 GHz = 37.2
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of a class kernel, from the `ncu --set full` captures whose
+# summaries are committed under profiles/ (a profiler number, quoted, never measured inside a timed run):
+# {workload: {class: (bytes, source)}}.  A dominant kernel without a capture reports "traffic": null.
+NCU_DRAM_BYTES = {
+    "cfg4_300atom_globular_2500bf": {
+        "(dp|pp)": (140.9e9, "profiles/r01_ncu_full_cfg4.md"),
+        "(ps|ss)": (3.77e9, "profiles/r01_ncu_full_cfg4.md"),
+    },
+}
 
 
 class ClockSampler:
@@ -246,7 +258,7 @@ def main():
         dom_tflops = cmf[dom] / (class_ms[dom] * 1e-3) / 1e12
         # roofline of the dominant kernel launch: algorithmic (model) FP64 flops of that class launch / its duration
         # measured live with CUDA events on the launching stream (adft_jk_stats.class_ms).  Bound: plain FP64 ALUs.
-        roofline = {"bound": "alu", "kernel": f"jk_kernel<{CLASS_NAMES[dom]}>", "kernel_ms": float(class_ms[dom]),
+        roofline = {"bound": "alu", "kernel": f"{'jk_rys_kernel' if CLASS_NAMES[dom] in RYS_CLASSES else 'jk_kernel'}<{CLASS_NAMES[dom]}>", "kernel_ms": float(class_ms[dom]),
                     "kernel_share_of_step": float(class_ms[dom] / ms_step), "kernel_model_flops": float(cmf[dom]),
                     "achieved": dom_tflops, "peak": peak, "unit": "TFLOP/s", "frac": dom_tflops / peak,
                     "whole_step_achieved": step_tflops, "whole_step_frac": step_tflops / peak,
@@ -254,6 +266,10 @@ def main():
                                    f"burst); nominal {NOMINAL_FP64_TFLOPS:.1f} TFLOP/s = 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz; "
                                    "MEASURED_PEAKS.json has no FP64 entry",
                     "traffic": None}
+        cap = NCU_DRAM_BYTES.get(WORKLOAD_NAMES[args.config], {}).get(CLASS_NAMES[dom])
+        if cap:
+            roofline["traffic"] = cap[0]
+            roofline["traffic_source"] = f"dram read+write bytes of one launch of this kernel, ncu --set full, {cap[1]}"
         out = {"metric": "screened_eri_quartets_per_s", "value": value, "unit": "quartets/s", "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",

@@ -111,7 +111,7 @@ adft_status_t adft_shellpairs_build(const adft_basis_t *basis, void *cuda_stream
  * is below prim_threshold (absolute, in sqrt(Hartree)); the largest primitive pair of a shell pair is always kept.
  * prim_threshold = 0 keeps every primitive pair (the plain definition, what the oracle evaluates).
  * adft_shellpairs_build uses ADFT_DEFAULT_PRIM_THRESHOLD.  Errors: negative or non-finite threshold -> INVALID_ARG. */
-#define ADFT_DEFAULT_PRIM_THRESHOLD 1e-20
+#define ADFT_DEFAULT_PRIM_THRESHOLD 1e-15
 adft_status_t adft_shellpairs_build_ex(const adft_basis_t *basis, double prim_threshold, void *cuda_stream,
                                        adft_shellpairs_t **out);
 

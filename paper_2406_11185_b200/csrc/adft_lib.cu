@@ -560,7 +560,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     ALLOC(p->d_AB, 3 * np * sizeof(double));
     ALLOC(p->d_pint, 5 * np * sizeof(int32_t));
     ALLOC(p->d_prim, 9 * npp * sizeof(double));
-    ALLOC(p->d_boys, (size_t)BOYS_NT * BOYS_NM * sizeof(double));
+    ALLOC(p->d_boys, (size_t)BOYS_ALLOC * sizeof(double));
     ALLOC(p->d_counters, 4 * NQCLASS * sizeof(unsigned long long));
     {
         // interpreter resources, only if some class that can occur lacks straight-line code
@@ -628,6 +628,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
                              cudaMemcpyHostToDevice, st));
     std::vector<double> boys;
     fill_boys_table(boys);
+    boys.resize(BOYS_ALLOC, 0.0);                 // second copy shifted by one double (128-bit loads of odd columns)
+    std::copy(boys.begin(), boys.begin() + BOYS_NT * BOYS_NM, boys.begin() + BOYS_ODD_SHIFT);
     TRY2(cudaMemcpyAsync(p->d_boys, boys.data(), boys.size() * sizeof(double), cudaMemcpyHostToDevice, st));
     TRY2(cudaStreamSynchronize(st));
 

@@ -159,7 +159,9 @@ def test_primitive_screening(api, orc):
     for st in (st0, st1, st2):
         assert st.quartets_kept == cnt["kept"]
     assert np.abs(J0 - Jo).max() <= TOL_ELEM and np.abs(K0 - Ko).max() <= TOL_ELEM
-    assert np.abs(J1 - J0).max() <= 1e-12 and np.abs(K1 - K0).max() <= 1e-12
+    # default threshold: the change must stay an order of magnitude inside the 1e-10 tolerance (measured on cfg 4:
+    # 2e-12, the same as the run-to-run spread of the atomics; R-11)
+    assert np.abs(J1 - J0).max() <= 1e-11 and np.abs(K1 - K0).max() <= 1e-11
     assert np.abs(J2 - J0).max() > 1e-10
     b = api.Basis.from_workload(w)
     for bad in (-1.0, float("nan"), float("inf")):
@@ -168,7 +170,7 @@ def test_primitive_screening(api, orc):
         assert e.value.status == 1
     sp = api.ShellPairs(b)
     nominal, kept, thr = sp.prim_counts()
-    assert kept < nominal and thr == 1e-20
+    assert kept < nominal and thr == 1e-15
     sp.close(); b.close()
 
 
@@ -239,3 +241,9 @@ def test_cfg2_sampled_parity(api, orc):
 def test_cfg3_sampled_parity(api, orc):
     """cfg 3 (f shells on the heavy atoms, d on the light ones): all 55 quartet classes."""
     sampled_parity(api, orc, W.make(3), nsamples=4, seed=3)
+
+
+def test_cfg4_sampled_parity(api, orc):
+    """cfg 4 (300 atoms, 2500 functions, tau = 1e-11): the workload and launch configuration bench.py times.
+    Equal per-class kept counts (6.17e9 quartets) and sampled J/K shell blocks against the definition."""
+    sampled_parity(api, orc, W.make(4), nsamples=3, seed=4)
