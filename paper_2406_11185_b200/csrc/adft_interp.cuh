@@ -28,6 +28,7 @@ struct InterpParams {
     double *scratch;                  // [nslots][stride]
     long long stride;                 // threads of the persistent grid
     unsigned long long *tile_counter; // zeroed before the launch
+    const double *boys_plain;         // F_m(T_k) table [BOYS_NT][BOYS_NM] (boys_scaled_rt)
 };
 
 __host__ __device__ inline int interp_ncart(int l) { return (l + 1) * (l + 2) / 2; }
@@ -168,7 +169,7 @@ __global__ void __launch_bounds__(128) jk_interp_kernel(const InterpParams q)
             const PrimPair bp = load_prim(p.t, sg.bra_prim_base + kb * sg.bra_n + i);
             for (int kk = 0; kk < sg.ket_K; ++kk) {
                 const PrimPair kp = load_prim(p.t, sg.ket_prim_base + kk * sg.ket_n + j);
-                interp_prim_quartet(pg, bp, kp, p.boys, S, A, st);
+                interp_prim_quartet(pg, bp, kp, q.boys_plain, S, A, st);
             }
         }
         // D blocks (weight folded in) and zeroed J/K blocks

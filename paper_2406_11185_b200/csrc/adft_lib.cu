@@ -245,7 +245,8 @@ struct adft_shellpairs {
     // device: pair table
     double *d_Q = nullptr, *d_AB = nullptr /* 3*npairs */, *d_prim = nullptr /* 9*nprimpairs */;
     int32_t *d_pint = nullptr /* 5*npairs: bfa,bfb,sha,shb,knom */;
-    double *d_boys = nullptr;
+    double *d_boys = nullptr;                 // F_m(T_k), [BOYS_NT][BOYS_NM] (interpreter)
+    double *d_boysp = nullptr;                // per-order Taylor tables [BOYS_MORD][BOYS_NT][BOYS_NC] (generated kernels)
     PairTable tab{};
     // per-build workspaces
     Segment *d_segs = nullptr, *h_segs = nullptr;
@@ -401,7 +402,7 @@ static void free_pairs(adft_shellpairs *p)
     if (!p) return;
     cudaFree(p->d_xyz); cudaFree(p->d_expo); cudaFree(p->d_coef); cudaFree(p->d_atom); cudaFree(p->d_nprim);
     cudaFree(p->d_off); cudaFree(p->d_Q); cudaFree(p->d_AB); cudaFree(p->d_prim); cudaFree(p->d_pint);
-    cudaFree(p->d_boys); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage); cudaFree(p->d_sink);
+    cudaFree(p->d_boys); cudaFree(p->d_boysp); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage); cudaFree(p->d_sink);
     cudaFree(p->d_blob); cudaFree(p->d_scratch); cudaFree(p->d_rys);
     if (p->h_segs) cudaFreeHost(p->h_segs);
     if (p->h_small) cudaFreeHost(p->h_small);
@@ -560,7 +561,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     ALLOC(p->d_AB, 3 * np * sizeof(double));
     ALLOC(p->d_pint, 5 * np * sizeof(int32_t));
     ALLOC(p->d_prim, 9 * npp * sizeof(double));
-    ALLOC(p->d_boys, (size_t)BOYS_ALLOC * sizeof(double));
+    ALLOC(p->d_boys, (size_t)BOYS_NT * BOYS_NM * sizeof(double));
+    ALLOC(p->d_boysp, (size_t)BOYS_MORD * BOYS_NT * BOYS_NC * sizeof(double));
     ALLOC(p->d_counters, 4 * NQCLASS * sizeof(unsigned long long));
     {
         // interpreter resources, only if some class that can occur lacks straight-line code
@@ -628,9 +630,18 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
                              cudaMemcpyHostToDevice, st));
     std::vector<double> boys;
     fill_boys_table(boys);
-    boys.resize(BOYS_ALLOC, 0.0);                 // second copy shifted by one double (128-bit loads of odd columns)
-    std::copy(boys.begin(), boys.begin() + BOYS_NT * BOYS_NM, boys.begin() + BOYS_ODD_SHIFT);
     TRY2(cudaMemcpyAsync(p->d_boys, boys.data(), boys.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    // per-order tables: a_j = F_{M+j}(T_k) / j!, j = 0..9  (Taylor coefficients of F_M about T_k in d = T_k - T)
+    std::vector<double> boysp((size_t)BOYS_MORD * BOYS_NT * BOYS_NC);
+    for (int M = 0; M < BOYS_MORD; ++M)
+        for (int k = 0; k < BOYS_NT; ++k) {
+            long double fact = 1.0L;
+            for (int j = 0; j < BOYS_NC; ++j) {
+                if (j > 0) fact *= (long double)j;
+                boysp[((size_t)M * BOYS_NT + k) * BOYS_NC + j] = (double)((long double)boys[(size_t)k * BOYS_NM + M + j] / fact);
+            }
+        }
+    TRY2(cudaMemcpyAsync(p->d_boysp, boysp.data(), boysp.size() * sizeof(double), cudaMemcpyHostToDevice, st));
     TRY2(cudaStreamSynchronize(st));
 
     // pass 1: records of ALL primitive pairs in bucket order, Schwarz bounds from the full contraction
@@ -640,7 +651,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
         if (s.n == 0) continue;
         const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
         if (ce.launch_schwarz && !ce.use_table) {
-            ce.launch_schwarz(p->tab, s.pair_base, s.prim_base, s.n, s.K, p->d_boys, p->d_Q, st);
+            ce.launch_schwarz(p->tab, s.pair_base, s.prim_base, s.n, s.K, p->d_boysp, p->d_Q, st);
         } else if (ce.use_rys && rys_schwarz_launcher(s.la, s.lb)) {
             TRY2(rys_schwarz_launcher(s.la, s.lb)(p->tab, p->rys, s.pair_base, s.prim_base, s.n, s.K, p->d_Q, st));
         } else {
@@ -851,7 +862,7 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         if (warps[qc] == 0) continue;
         JKParams prm{};
         prm.t = p->tab; prm.segs = p->d_segs + seg_off[qc]; prm.nsegs = (int)plan[qc].size(); prm.total_warps = warps[qc];
-        prm.D = D; prm.J = Jw; prm.K = Kw; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boys;
+        prm.D = D; prm.J = Jw; prm.K = Kw; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boysp;
         prm.counters = p->d_counters + 4 * qc; prm.zero = 0;
         CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
         const ClassEntry &ce = class_table()[qc];
@@ -862,6 +873,7 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
             ip.jk = prm; ip.prog = make_prog(ce, p->d_blob, false);
             ip.scratch = p->d_scratch; ip.stride = p->scratch_threads;
             ip.tile_counter = p->d_counters + 4 * qc + 3;
+            ip.boys_plain = p->d_boys;
             const long long want = (warps[qc] + 3) / 4;
             jk_interp_kernel<<<(unsigned)std::min<long long>(want, p->interp_blocks), 128, 0, st>>>(ip);
         } else {
