@@ -99,6 +99,24 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def reduce_max_over_ranks(values, world, device="cpu"):
+    """Timing of a multi-rank run = the slowest rank: element-wise MAX of `values` over all ranks (all-reduce on the
+    initialised process group: NCCL with a CUDA `device` in the benchmark, gloo on the CPU in tests/)."""
+    if world == 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def job_value(kept_per_replica, world, ms_per_step):
+    """Whole-job throughput of `world` independent replicas ("replicas only"): every rank builds
+    J and K of the same workload, so the job processes world * kept quartets in the time of the slowest rank."""
+    return world * kept_per_replica / (ms_per_step * 1e-3)
+
+
 def oracle_sample(w, seconds_target, seed=7):
     """Time the oracle, as it stands, on a bounded sample of the workload: J and K shell blocks evaluated from the
     definition with the same screen (oracle.jk_block) for random shell pairs until ~seconds_target of wall time."""
@@ -224,12 +242,9 @@ def main():
     region_ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
     ms_step = float(np.mean(step_ms))
-    if world > 1:
-        t = torch.tensor([ms_step, region_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step, region_ms = float(t[0]), float(t[1])
+    ms_step, region_ms = reduce_max_over_ranks([ms_step, region_ms], world, "cuda")
     kept = int(stats.quartets_kept)
-    value = world * kept / (ms_step * 1e-3)
+    value = job_value(kept, world, ms_step)
 
     # end to end: host buffers through adft_jk_build_host (H2D of D, D2H of J and K inside the timed region)
     Dh = torch.from_numpy(w.D).pin_memory(); Jh = torch.empty(N, N, dtype=torch.float64).pin_memory()
@@ -242,11 +257,8 @@ def main():
         sp.jk_build_host(Dh.numpy(), Jh.numpy(), Kh.numpy(), w.tau)
         chk = float(Jh[0, 0])                         # host read of the result
     e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t[0])
-    e2e_value = world * kept / (e2e_ms * 1e-3)
+    e2e_ms = reduce_max_over_ranks([e2e_ms], world, "cuda")[0]
+    e2e_value = job_value(kept, world, e2e_ms)
     assert np.isfinite(chk)
 
     if rank == 0:
