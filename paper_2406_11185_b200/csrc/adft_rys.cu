@@ -31,18 +31,21 @@ static cudaError_t run_sw(const PairTable &t, const RysTable &rt, int pair_base,
     return launch_schwarz_rys<C>(t, rt, pair_base, prim_base, n, K, Qout, 2 * sms, st);
 }
 
+// X(la, lb, lc, ld, NCH): NCH = number of cd chunks = thread groups per quartet.  Phase 2 is bound by shared-memory
+// bandwidth (3*(lc+1)(ld+1) loads per 2*CH FP64 instructions per batch item), so NCH is as small as the register file
+// allows (CH = ceil(NC*ND/NCH) contracted integrals per thread, <= 50).
 #define ADFT_RYS_CLASSES(X) \
-    X(3, 1, 3, 1, 4)        \
+    X(3, 1, 3, 1, 2)        \
     X(3, 3, 1, 1, 1)        \
-    X(3, 2, 2, 1, 2)        \
+    X(3, 2, 2, 1, 1)        \
     X(3, 3, 3, 0, 1)        \
-    X(3, 1, 2, 2, 4)        \
-    X(3, 2, 3, 1, 2)        \
-    X(3, 3, 2, 1, 2)        \
-    X(3, 2, 2, 2, 2)        \
-    X(3, 3, 3, 1, 2)        \
+    X(3, 1, 2, 2, 2)        \
+    X(3, 2, 3, 1, 1)        \
+    X(3, 3, 2, 1, 1)        \
+    X(3, 2, 2, 2, 1)        \
+    X(3, 3, 3, 1, 1)        \
     X(3, 2, 3, 2, 2)        \
-    X(3, 3, 2, 2, 2)        \
+    X(3, 3, 2, 2, 1)        \
     X(3, 3, 3, 2, 2)        \
     X(3, 3, 3, 3, 2)
 
@@ -57,7 +60,7 @@ rys_jk_fn rys_jk_launcher(int la, int lb, int lc, int ld)
 
 rys_sw_fn rys_schwarz_launcher(int la, int lb)
 {
-    if (la == 3 && lb == 1) return run_sw<RysCfg<3, 1, 3, 1, 4>>;
+    if (la == 3 && lb == 1) return run_sw<RysCfg<3, 1, 3, 1, 2>>;
     if (la == 3 && lb == 2) return run_sw<RysCfg<3, 2, 3, 2, 2>>;
     if (la == 3 && lb == 3) return run_sw<RysCfg<3, 3, 3, 3, 2>>;
     return nullptr;

@@ -103,9 +103,10 @@ struct RysCfg {
     static constexpr int PADCD = NKL | 1;                          // odd stride: the (i,j) slots fall in distinct banks
     static constexpr int AXSZ = (LA + 1) * (LB + 1) * PADCD;
     static constexpr int ITEMSZ = 3 * AXSZ;                        // doubles per (primitive quartet, root)
-    static constexpr int SMEM_BUDGET = ITEMSZ * 8 > 4096 ? 196 * 1024 : 72 * 1024;
+    // shared memory per block: one big block per SM for the largest classes, several small blocks per SM otherwise
+    static constexpr int SMEM_BUDGET = ITEMSZ * 8 > 4096 ? 196 * 1024 : (NT <= 64 ? 32 * 1024 : 64 * 1024);
     static constexpr int BATCH_S = SMEM_BUDGET / (ITEMSZ * 8);
-    static constexpr int BATCH = BATCH_S < NT / 3 ? BATCH_S : NT / 3;
+    static constexpr int BATCH = BATCH_S < 64 ? BATCH_S : 64;      // phase 1 strides over 3*BATCH units with NT threads
     static constexpr size_t SMEM_BYTES = (size_t)BATCH * ITEMSZ * 8;
 };
 
