@@ -247,3 +247,42 @@ def test_cfg4_sampled_parity(api, orc):
     """cfg 4 (300 atoms, 2500 functions, tau = 1e-11): the workload and launch configuration bench.py times.
     Equal per-class kept counts (6.17e9 quartets) and sampled J/K shell blocks against the definition."""
     sampled_parity(api, orc, W.make(4), nsamples=3, seed=4)
+
+
+def test_degenerate_inputs(api, orc):
+    """The degenerate cases of the path: one basis function; a threshold that screens every quartet out; D = 0;
+    a shell with 1 primitive next to shells with the deepest contraction the configs use (6)."""
+    import torch
+    # (1) a single s function: one pair, one quartet, J = K = D (ss|ss)
+    w1 = W.make_custom(np.zeros((1, 3)), [(0, 0)], seed=11, nprim=3)
+    check_full(api, orc, w1, tau=0.0)
+    J, K, st, Q = api.jk(w1, 0.0)
+    assert st.quartets_unique == 1 and st.quartets_kept == 1 and J.shape == (1, 1)
+    assert J[0, 0] == pytest.approx(w1.D[0, 0] * Q[0, 0] ** 2, rel=1e-13) and K[0, 0] == pytest.approx(J[0, 0], rel=1e-13)
+    # (2) everything screened out: J = K = 0 exactly, zero kept quartets, no class kernel has anything to do
+    w = W.make(1)
+    J, K, st, Q = api.jk(w, tau=1e30)
+    assert st.quartets_kept == 0 and st.prim_quartets == 0
+    assert not J.any() and not K.any()
+    bs = orc.basis_from_workload(w)
+    assert orc.count(bs, orc.schwarz(bs), orc.dmax(w.D), 1e30)["kept"] == 0
+    # (3) D = 0: Dmax = 0, so every product is 0: kept iff tau == 0; the results are exact zeros either way
+    b = api.Basis.from_workload(w); sp = api.ShellPairs(b)
+    D0 = torch.zeros(w.nbf, w.nbf, dtype=torch.float64, device="cuda")
+    Jt = torch.full_like(D0, 1.0); Kt = torch.full_like(D0, 1.0)
+    sp.jk_build(D0, Jt, Kt, w.tau); torch.cuda.synchronize()
+    assert sp.stats().quartets_kept == 0 and not Jt.any().item() and not Kt.any().item()
+    sp.jk_build(D0, Jt, Kt, 0.0); torch.cuda.synchronize()
+    assert sp.stats().quartets_kept == sp.stats().quartets_unique and not Jt.any().item() and not Kt.any().item()
+    sp.close(); b.close()
+    # (4) contraction depths 1 and 6 side by side (sublists of different depth meet in one class launch)
+    atoms = np.array([[0.0, 0.0, 0.0], [1.1, 0.3, -0.4], [-0.7, 1.2, 0.6]])
+    for nprim_mix in ((1, 6, 1, 6), (6, 1, 6, 1)):
+        rng = np.random.default_rng(5)
+        s_l = [2, 1, 0, 2]; s_atom = [0, 1, 2, 2]
+        s_np = np.array(nprim_mix, np.int32); s_off = np.concatenate([[0], np.cumsum(s_np)[:-1]]).astype(np.int32)
+        e = np.exp(rng.uniform(np.log(0.2), np.log(30.0), int(s_np.sum()))); c = rng.uniform(0.1, 1.0, int(s_np.sum()))
+        nbf = sum((l + 1) * (l + 2) // 2 for l in s_l)
+        C = rng.normal(size=(nbf, 3))
+        wm = W.Workload("mix", atoms, np.array(s_atom, np.int32), np.array(s_l, np.int32), s_np, s_off, e, c, C @ C.T / 3, 0.0)
+        check_full(api, orc, wm, tau=0.0)
