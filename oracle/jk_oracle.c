@@ -18,7 +18,9 @@
  *
  * Pins (tests/test_oracle_*.py): P1 Boys, P2-P4 closed forms, P5/P5b contraction+normalisation+J/K,
  * P6 one-centre high-L closed form, P7 derivative identity, P8 axis permutations, P9 symmetry,
- * P10 Schwarz, P11 positivity, P12 brute force, P13 long-double rerun, P14 screening bounds.
+ * P10 Schwarz, P11 positivity, P12 brute force, P13 long-double rerun, P14 screening bounds,
+ * P15 order independence of the recurrence centre (R-22: the integral core builds the recurrences on the
+ * centre nearest to each primitive pair's product centre, eri_core.inc.c).
  * No function here is "parity unpinned".
  */
 #include <math.h>

@@ -323,9 +323,10 @@ def test_p13_long_double_agreement(orc):
 
 
 def test_p13_documented_hrr_cancellation_case(orc):
-    """DESIGN.md R-19: cfg 1 shells (35, 23) -- a diffuse p shell 8.5 bohr from a tight d shell.  The plain fp64 core
-    loses digits there (HRR shifts angular momentum onto the tight shell); the long-double core, which the oracle
-    proper uses, does not depend on the order the two shells are given in."""
+    """DESIGN.md R-19 / R-22: cfg 1 shells (35, 23) -- a diffuse p shell 8.5 bohr from a tight d shell.  Before R-22 the
+    single-orientation fp64 core lost digits there (the HRR shifted angular momentum onto the tight shell); with the
+    recurrences built on the centre nearest to each primitive pair's product centre neither core depends on the order the
+    two shells are given in, and the Schwarz table (long-double core) matches the block's largest diagonal element."""
     w = W.make(1)
     bs = orc.basis_from_workload(w)
     A, B = 35, 23
