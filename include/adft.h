@@ -79,9 +79,12 @@ typedef struct {
     int32_t reserved;
 } adft_jk_stats_t;
 
+#define ADFT_MAX_NPRIM 32        /* largest contraction depth of one shell */
+
 /* Copy and validate a basis.  All input arrays are HOST memory and are copied; the caller may free them on return.
  *   atom_xyz_bohr [natoms*3], shells [nshells], exponents / coefficients [sum of nprim] (indexed via prim_offset).
- * Errors: NULL / sizes <= 0 / atom index out of range / nprim < 1 / exponent <= 0 or non-finite -> INVALID_ARG;
+ * Errors: NULL / sizes <= 0 / atom index out of range / nprim < 1 or > ADFT_MAX_NPRIM / exponent <= 0 or non-finite
+ *         -> INVALID_ARG;
  *         l outside 0..3 -> UNSUPPORTED_L.  *out is written only on success.  Needs no GPU. */
 adft_status_t adft_basis_create(int32_t natoms, const double *atom_xyz_bohr,
                                 int32_t nshells, const adft_shell_t *shells,

@@ -101,6 +101,7 @@ static int schwarz_slots_of(const ClassEntry &e)
     } while (0)
 
 static inline int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+#define ADFT_MAX_PRIM_PAIRS (ADFT_MAX_NPRIM * ADFT_MAX_NPRIM)     // primitive pairs of one shell pair the sorter holds
 
 // ------------------------------------------------------------------ small kernels
 // (a2) primitive screening estimate of primitive pair (alpha on A, beta on B) of a shell pair with angular momenta
@@ -152,13 +153,27 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int la, in
         }
     if (kcount) { kcount[g] = cnt > 0 ? cnt : 1; return; }
     const double c0 = 5.9149671727956128778;     // sqrt(2) * pi^(5/4)
-    int k = 0;
+    // The surviving primitive pairs are stored in DESCENDING order of zeta = alpha + beta (ties: nominal order).  All
+    // lanes of a warp walk primitive lists of the same length; with the lists ranked by exponent the Boys argument
+    // T = rho |PQ|^2 of step (kb, kk) is large in most lanes together (tight x tight first) or small together, so the
+    // T < / >= switch branches of boys_scaled are taken warp-uniformly more often.
+    int order[ADFT_MAX_PRIM_PAIRS];
+    double okey[ADFT_MAX_PRIM_PAIRS];
+    int nk = 0;
     for (int ia = 0; ia < npa; ++ia)
         for (int ib = 0; ib < npb; ++ib) {
             const double a = expo[sh_off[sa] + ia], b = expo[sh_off[sb] + ib];
+            const bool keep = cnt > 0 ? (prim_pair_estimate(a, b, coef[sh_off[sa] + ia], coef[sh_off[sb] + ib], AB2, la, lb) >= thr)
+                                      : (ia * npb + ib == best);
+            if (!keep || nk >= ADFT_MAX_PRIM_PAIRS) continue;
+            int pos = nk++;
+            while (pos > 0 && okey[pos - 1] < a + b) { okey[pos] = okey[pos - 1]; order[pos] = order[pos - 1]; --pos; }
+            okey[pos] = a + b; order[pos] = ia * npb + ib;
+        }
+    for (int k = 0; k < nk; ++k) {
+            const int ia = order[k] / npb, ib = order[k] % npb;
+            const double a = expo[sh_off[sa] + ia], b = expo[sh_off[sb] + ib];
             const double da = coef[sh_off[sa] + ia], db = coef[sh_off[sb] + ib];
-            const bool keep = cnt > 0 ? (prim_pair_estimate(a, b, da, db, AB2, la, lb) >= thr) : (ia * npb + ib == best);
-            if (!keep) continue;
             const double z = a + b, iz = 1.0 / z;
             const double px = (a * Ax + b * Bx) * iz, py = (a * Ay + b * By) * iz, pz = (a * Az + b * Bz) * iz;
             const int idx = prim_base + k * n + j;
@@ -166,8 +181,7 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int la, in
             Px[idx] = px;  Py[idx] = py;  Pz[idx] = pz;
             PAx[idx] = px - Ax;  PAy[idx] = py - Ay;  PAz[idx] = pz - Az;
             cc[idx] = c0 * da * db * exp(-a * b * iz * AB2) * iz;
-            ++k;
-        }
+    }
 }
 
 // (a3) max|D| with non-finite detection.  out[0] = bit pattern of the max (non-negative doubles order like
@@ -312,7 +326,7 @@ extern "C" adft_status_t adft_basis_create(int32_t natoms, const double *xyz, in
             set_error("adft_basis_create: shell " + std::to_string(s) + " has l=" + std::to_string(sh.l) + " (supported 0..3)");
             delete b; return ADFT_ERR_UNSUPPORTED_L;
         }
-        if (sh.atom < 0 || sh.atom >= natoms || sh.nprim < 1 || sh.prim_offset < 0) {
+        if (sh.atom < 0 || sh.atom >= natoms || sh.nprim < 1 || sh.nprim > ADFT_MAX_NPRIM || sh.prim_offset < 0) {
             set_error("adft_basis_create: shell " + std::to_string(s) + " has a bad atom index, nprim or offset");
             delete b; return ADFT_ERR_INVALID_ARG;
         }
