@@ -101,7 +101,10 @@ struct RysCfg {
     static constexpr int CH = (NCD + NCH - 1) / NCH;               // cd component pairs per thread
     static constexpr int NKL = (LC + 1) * (LD + 1);
     static constexpr int PADCD = NKL | 1;                          // odd stride: the (i,j) slots fall in distinct banks
-    static constexpr int AXSZ = (LA + 1) * (LB + 1) * PADCD;
+    // doubles per (item, axis), odd: in phase 1 the 16 lanes of a 64-bit shared-memory wavefront write the same slot of
+    // 16 consecutive (item, axis) units, AXSZ doubles apart; an even AXSZ folds them onto a few banks (ncu, (fd|dp) with
+    // AXSZ = 84: 31% of all shared-memory wavefronts were bank-conflict replays, L1/TEX at 91% of peak)
+    static constexpr int AXSZ = ((LA + 1) * (LB + 1) * PADCD) | 1;
     static constexpr int ITEMSZ = 3 * AXSZ;                        // doubles per (primitive quartet, root)
     // shared memory per block: one big block per SM for the largest classes, several small blocks per SM otherwise
     static constexpr int SMEM_BUDGET = ITEMSZ * 8 > 4096 ? 196 * 1024 : (NT <= 64 ? 32 * 1024 : 64 * 1024);
