@@ -111,6 +111,7 @@ struct RysCfg {
     static constexpr int BATCH_S = SMEM_BUDGET / (ITEMSZ * 8);
     static constexpr int BATCH = BATCH_S < 64 ? BATCH_S : 64;      // phase 1 strides over 3*BATCH units with NT threads
     static constexpr size_t SMEM_BYTES = (size_t)BATCH * ITEMSZ * 8;
+    static constexpr int MINB = NT <= 64 ? 6 : (NT <= 128 ? 3 : 1);   // resident blocks per SM asked of the register allocator
 };
 
 // phase 1: the 2-D integrals of one (primitive quartet, root, axis), all (i<=la, j<=lb, k<=lc, l<=ld), to `out`
@@ -386,7 +387,7 @@ __device__ __forceinline__ void rys_quartet(const PairTable &t, const RysTable &
 }
 
 template <class C>
-__global__ void __launch_bounds__(C::NT, 1) jk_rys_kernel(const JKParams p, const RysTable rt, unsigned long long *tile_counter)
+__global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p, const RysTable rt, unsigned long long *tile_counter)
 {
     extern __shared__ double sm[];
     __shared__ long long s_tile;
