@@ -148,6 +148,21 @@ def jk(bs: Basis, D, tau: float, Q=None):
     return J, K, {"unique": int(counts[0]), "kept": int(counts[1]), "prim": int(counts[2]), "per_class": cc}
 
 
+def jk_range(bs: Basis, D, tau: float, Q, pab_lo: int, pab_hi: int):
+    """orc_jk's loop over the bra pairs pab = A(A+1)/2+B in [pab_lo, pab_hi) only: long double partial J, K and the
+    counts of that range (the partial results of disjoint ranges covering all pairs add up to jk()'s result)."""
+    D = np.ascontiguousarray(D, np.float64)
+    N = bs.nbf
+    J = np.zeros((N, N), dtype=np.longdouble); K = np.zeros((N, N), dtype=np.longdouble)
+    counts = np.zeros(3, dtype=np.int64); cc = np.zeros(55, dtype=np.int64)
+    rc = lib().orc_jk_range(*bs.args(), _p(D, C.c_double), C.c_double(tau), _p(np.ascontiguousarray(Q, np.float64), C.c_double),
+                            C.c_int64(pab_lo), C.c_int64(pab_hi), _p(J, C.c_longdouble), _p(K, C.c_longdouble),
+                            _p(counts, C.c_int64), _p(cc, C.c_int64))
+    if rc:
+        raise ValueError(f"orc_jk_range rc={rc}")
+    return J, K, {"unique": int(counts[0]), "kept": int(counts[1]), "prim": int(counts[2]), "per_class": cc}
+
+
 def count(bs: Basis, Q, Dmax: float, tau: float):
     counts = np.zeros(3, dtype=np.int64); cc = np.zeros(55, dtype=np.int64)
     Q = np.ascontiguousarray(Q, np.float64)

@@ -234,12 +234,11 @@ static int qclass(int la, int lb, int lc, int ld)
     return X * (X + 1) / 2 + Y;
 }
 
-/* ---- exported: screened, 8-fold-symmetric J/K (the oracle proper) ----
- * Q may be NULL (computed here) or a caller-supplied table from orc_schwarz.
- * counts[0] = unique quartets before screening, counts[1] = kept, counts[2] = primitive quartets in kept;
- * class_counts[55] = kept per class.  J, K: full symmetric [nbf*nbf], overwritten. */
-int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J, double *K,
-           int64_t *counts, int64_t *class_counts)
+/* The loop of orc_jk restricted to bra pairs pab in [pab_lo, pab_hi): long double partial sums Jt, Kt [nbf*nbf]
+ * (overwritten) and the counts of that range.  Summing the partial results of disjoint ranges that cover
+ * [0, npair) gives orc_jk's result; tests/golden/make_golden.py uses this to checkpoint the hours-long full runs. */
+static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, int64_t pab_lo, int64_t pab_hi,
+                    long double *Jt, long double *Kt, int64_t *counts, int64_t *class_counts)
 {
     basis_t b = mk_basis(BASIS_PASS);
     if (check_basis(&b)) return check_basis(&b);
@@ -251,8 +250,9 @@ int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J
     else { int e = orc_schwarz(BASIS_PASS, Q); if (e) return e; }
     const double Dmax = dmax_of(D, (size_t)N * N);
     const int64_t npair = (int64_t)nshells * (nshells + 1) / 2;
-    long double *Jt = (long double *)calloc((size_t)N * N, sizeof(long double));
-    long double *Kt = (long double *)calloc((size_t)N * N, sizeof(long double));
+    if (pab_lo < 0) pab_lo = 0;
+    if (pab_hi > npair) pab_hi = npair;
+    for (size_t i = 0; i < (size_t)N * N; ++i) Jt[i] = Kt[i] = 0;
     int64_t n_all = 0, n_kept = 0, n_prim = 0;
     int64_t cc[55]; memset(cc, 0, sizeof cc);
     int err = 0;
@@ -269,7 +269,7 @@ int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J
             err = -3;
         } else {
 #pragma omp for schedule(dynamic, 1)
-            for (int64_t pab = npair - 1; pab >= 0; --pab) {
+            for (int64_t pab = pab_hi - 1; pab >= pab_lo; --pab) {
                 /* decode pab = A(A+1)/2 + B */
                 int A = (int)((sqrt(8.0 * (double)pab + 1.0) - 1.0) / 2.0);
                 while ((int64_t)A * (A + 1) / 2 > pab) --A;
@@ -319,11 +319,36 @@ int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J
         }
         core_scratch_free(&s); free(blk); free(Jp); free(Kp);
     }
-    for (size_t i = 0; i < (size_t)N * N; ++i) { J[i] = (double)Jt[i]; K[i] = (double)Kt[i]; }
     if (counts) { counts[0] = n_all; counts[1] = n_kept; counts[2] = n_prim; }
     if (class_counts) memcpy(class_counts, cc, sizeof cc);
-    free(Jt); free(Kt); free(Q); free(bo);
+    free(Q); free(bo);
     return err;
+}
+
+/* ---- exported: screened, 8-fold-symmetric J/K (the oracle proper) ----
+ * Q may be NULL (computed here) or a caller-supplied table from orc_schwarz.
+ * counts[0] = unique quartets before screening, counts[1] = kept, counts[2] = primitive quartets in kept;
+ * class_counts[55] = kept per class.  J, K: full symmetric [nbf*nbf], overwritten. */
+int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J, double *K,
+           int64_t *counts, int64_t *class_counts)
+{
+    size_t N = 0;
+    for (int s = 0; s < nshells; ++s) N += (l[s] >= 0 && l[s] <= LMAX_SHELL) ? NCART(l[s]) : 0;
+    long double *Jt = (long double *)calloc(N * N + 1, sizeof(long double));
+    long double *Kt = (long double *)calloc(N * N + 1, sizeof(long double));
+    if (!Jt || !Kt) { free(Jt); free(Kt); return -3; }
+    int err = jk_range(BASIS_PASS, D, tau, Qin, 0, (int64_t)nshells * (nshells + 1) / 2, Jt, Kt, counts, class_counts);
+    if (err == 0)
+        for (size_t i = 0; i < N * N; ++i) { J[i] = (double)Jt[i]; K[i] = (double)Kt[i]; }
+    free(Jt); free(Kt);
+    return err;
+}
+
+/* ---- exported: orc_jk's loop over the bra pairs pab in [pab_lo, pab_hi) only, long double partial sums out ---- */
+int orc_jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, int64_t pab_lo, int64_t pab_hi,
+                 long double *Jpart, long double *Kpart, int64_t *counts, int64_t *class_counts)
+{
+    return jk_range(BASIS_PASS, D, tau, Qin, pab_lo, pab_hi, Jpart, Kpart, counts, class_counts);
 }
 
 /* ---- exported: kept-quartet counts only (no integrals), same loop and rule as orc_jk ---- */
