@@ -128,16 +128,28 @@ def oracle_sample(w, seconds_target, seed=7):
     dm = oracle.dmax(w.D)
     rng = np.random.default_rng(seed)
     nq = npq = nblk = 0
+    blocks = []
     t0 = time.perf_counter()
     while True:
         A, B = (int(x) for x in rng.integers(0, bs.nshells, size=2))
-        _, _, (q, p) = oracle.jk_block(bs, w.D, w.tau, Q, dm, A, B, with_work=True)
+        Jb, Kb, (q, p) = oracle.jk_block(bs, w.D, w.tau, Q, dm, A, B, with_work=True)
+        blocks.append((A, B, Jb, Kb))
         nq += q; npq += p; nblk += 1
         el = time.perf_counter() - t0
         if el >= seconds_target or nblk >= 4000:
             break
     return {"quartets": nq, "prim_quartets": npq, "seconds": el, "blocks": nblk, "schwarz_seconds": t_q,
-            "threads": oracle.num_threads()}
+            "threads": oracle.num_threads(), "block_values": blocks, "bf_off": bs.bf_off}
+
+
+def sample_max_abs_err(smp, J, K):
+    """Largest |J_gpu - J_oracle|, |K_gpu - K_oracle| over the oracle's sampled shell blocks (host arrays J, K)."""
+    o = smp["bf_off"]
+    worst = 0.0
+    for (A, B, Jb, Kb) in smp["block_values"]:
+        worst = max(worst, float(np.abs(J[o[A]:o[A + 1], o[B]:o[B + 1]] - Jb).max()),
+                    float(np.abs(K[o[A]:o[A + 1], o[B]:o[B + 1]] - Kb).max()))
+    return worst
 
 
 def run_reference(args, rank, world):
@@ -250,7 +262,7 @@ def main():
     Dh = torch.from_numpy(w.D).pin_memory(); Jh = torch.empty(N, N, dtype=torch.float64).pin_memory()
     Kh = torch.empty(N, N, dtype=torch.float64).pin_memory()
     e2e_steps = max(1, min(args.steps, 2))
-    sp.jk_build_host(Dh.numpy(), Jh.numpy(), Kh.numpy(), w.tau) if args.config <= 2 else None
+    sp.jk_build_host(Dh.numpy(), Jh.numpy(), Kh.numpy(), w.tau)      # untimed: allocates the library's staging buffers
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
@@ -293,11 +305,16 @@ def main():
                           "prim_quartets_evaluated": int(stats.prim_quartets_evaluated), "parallelism": "replicas" if world > 1 else "1gpu",
                           "l2": "flushed between iterations (256 MiB write); pair table + D/J/K exceed L2",
                           "shellpairs_build_s": t_pairs},
-               "jk_build_ms": ms_step, "region_ms": region_ms,
+               "jk_build_ms": ms_step, "jk_build_ms_min": float(np.min(step_ms)), "jk_build_ms_median": float(np.median(step_ms)),
+               "region_ms": region_ms,
                "prim_quartets_per_s": world * int(stats.prim_quartets) / (ms_step * 1e-3),
                "prim_quartets_evaluated_per_s": world * int(stats.prim_quartets_evaluated) / (ms_step * 1e-3),
                "model_tflops": step_tflops, "fp64_peak_fraction": step_tflops / peak,
                "phase_ms": {"dmax": stats.ms_dmax, "plan": stats.ms_plan, "eri": stats.ms_eri, "finalize": stats.ms_finalize},
+               # the two HBM-bound phases against the measured copy bandwidth (MEASURED_PEAKS.json: 6496 GB/s on this pool):
+               # finalise reads and writes J and K once (4 N^2 doubles); Dmax includes the 16-byte D2H and the host sync
+               "phase_gbps": {"finalize": 4.0 * N * N * 8 / (stats.ms_finalize * 1e-3) / 1e9 if stats.ms_finalize > 0 else None,
+                              "dmax": N * N * 8 / (stats.ms_dmax * 1e-3) / 1e9 if stats.ms_dmax > 0 else None},
                "class_ms": {CLASS_NAMES[i]: round(float(class_ms[i]), 3) for i in range(55) if cq[i]},
                "class_model_tflops": {CLASS_NAMES[i]: round(float(cmf[i] / (class_ms[i] * 1e-3) / 1e12), 2)
                                       for i in range(55) if cq[i] and class_ms[i] > 0},
@@ -307,8 +324,9 @@ def main():
                "gpu_launches": int(stats.kernel_launches) * args.steps, "clocks": clocks}
         if not args.no_cpu_baseline:
             smp = oracle_sample(w, args.cpu_seconds)
+            err = sample_max_abs_err(smp, J.cpu().numpy(), K.cpu().numpy())      # the J, K of the timed builds
             out["cpu_baseline"] = {"value": smp["quartets"] / smp["seconds"], "unit": "quartets/s", "cores": smp["threads"],
-                                   "kind": "oracle",
+                                   "kind": "oracle", "max_abs_err": err,
                                    "sample": f"{smp['blocks']} random J+K shell blocks of the same workload evaluated from "
                                              f"the definition with the same screen (oracle.jk_block), {smp['seconds']:.1f} s, "
                                              f"{smp['quartets']} shell quartets / {smp['prim_quartets']} primitive quartets",

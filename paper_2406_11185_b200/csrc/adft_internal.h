@@ -23,16 +23,14 @@ struct ClassEntry {
                            double *Qout, cudaStream_t st) = nullptr;
     int la = 0, lb = 0, lc = 0, ld = 0;
     int vrr_ops = 0, hrr_ops = 0, nint = 0;   // FP64 instruction counts from the generator
-    const char *impl = "none";                // "straightline" | "table"
-    const int32_t *prog = nullptr;            // host copy of the class's table program (generated/programs.bin), if any
-    int64_t prog_off = 0;                     // its offset in the blob (int32 units)
-    bool use_table = false;                   // this class runs through the interpreter kernels (adft_interp.cuh)
+    const char *impl = "none";                // "straightline" | "rys"
     bool use_rys = false;                     // this class runs through the block-cooperative Rys kernels (adft_rys.cuh)
 };
 
 // Rys kernels (adft_rys.cu): launchers per class, nullptr where none is instantiated
 struct RysTable;
-typedef cudaError_t (*rys_jk_fn)(const JKParams &p, const RysTable &rt, unsigned long long *tile_counter, cudaStream_t st);
+typedef cudaError_t (*rys_jk_fn)(const JKParams &p, const RysTable &rt, unsigned long long *tile_counter, cudaStream_t st,
+                                 bool want_j, bool want_k);
 typedef cudaError_t (*rys_sw_fn)(const PairTable &t, const RysTable &rt, int pair_base, int prim_base, int n, int K,
                                  double *Qout, cudaStream_t st);
 rys_jk_fn rys_jk_launcher(int la, int lb, int lc, int ld);

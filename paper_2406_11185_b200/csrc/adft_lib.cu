@@ -7,8 +7,9 @@
 #include <cstring>
 #include <numeric>
 
+#include <mutex>
+
 #include "adft_internal.h"
-#include "adft_interp.cuh"
 #include "adft_rys.cuh"
 
 namespace adft {
@@ -18,77 +19,35 @@ void set_error(const std::string &msg) { g_last_error = msg; }
 
 static ClassEntry g_classes[NQCLASS];
 ClassEntry *class_table() { return g_classes; }
-static bool g_registered = false;
+static std::once_flag g_register_once;
 
 }  // namespace adft
-// table programs of every class (generated/programs.bin, linked in through generated/programs_blob.S)
-extern "C" const int32_t adft_prog_blob[];
-extern "C" const int32_t adft_prog_blob_end[];
 // Rys root/weight tables (generated/rys_tables.bin from csrc/gen/gen_rys.py, linked in through generated/rys_blob.S)
 extern "C" const double adft_rys_blob[];
 extern "C" const double adft_rys_blob_end[];
 namespace adft {
 
-// program header fields (gen_eri.py pack_program)
-enum { PH_MAGIC = 0, PH_LA = 1, PH_LB = 2, PH_LC = 3, PH_LD = 4, PH_NVRR = 5, PH_NVSLOTS = 6, PH_NACC = 7, PH_NHRR = 8,
-       PH_NHSLOTS = 9, PH_NOUT = 10, PH_MMAX = 11, PH_VRR_OPS = 12, PH_HRR_OPS = 13, PH_NINT = 14, PH_NHRR_DIAG = 15,
-       PH_NHSLOTS_DIAG = 16, PH_NOUT_DIAG = 17, PH_OFF_VRR = 18, PH_OFF_HRR = 19, PH_OFF_DIAG = 20, PH_TOTAL = 21 };
-
+// Fill the class table once per process: the generated straight-line classes register themselves (generated/registry.cu);
+// every other class of generated/class_meta.inc (angular momenta and the generator's FP64 instruction counts, used for
+// the model flops) runs through the block-cooperative Rys kernels.
 static void ensure_registered()
 {
-    if (g_registered) return;
-    register_all_classes();
-    // classes without generated straight-line code run through the interpreter; ADFT_FORCE_TABLE=1 (tests) sends
-    // every class there
-    const char *force = getenv("ADFT_FORCE_TABLE");
-    const bool force_table = force && force[0] == '1';
-    for (int qc = 0; qc < NQCLASS; ++qc) {
-        const int32_t off = adft_prog_blob[2 * qc], len = adft_prog_blob[2 * qc + 1];
-        if (len <= 0) continue;
-        const int32_t *pr = adft_prog_blob + off;
-        if (pr[PH_MAGIC] != 0x41444654 || pr[PH_TOTAL] != len) continue;
-        ClassEntry &e = g_classes[qc];
-        e.prog = pr;
-        e.prog_off = off;
-        const char *norys = getenv("ADFT_NO_RYS");
-        const bool have_rys = rys_jk_launcher(pr[PH_LA], pr[PH_LB], pr[PH_LC], pr[PH_LD]) != nullptr &&
-                              !(norys && norys[0] == '1');
-        if (!e.launch_jk || force_table) {
-            e.use_rys = have_rys && !force_table;
-            e.use_table = !e.use_rys;
-            e.impl = e.use_rys ? "rys" : "table";
-            e.la = pr[PH_LA]; e.lb = pr[PH_LB]; e.lc = pr[PH_LC]; e.ld = pr[PH_LD];
-            e.vrr_ops = pr[PH_VRR_OPS]; e.hrr_ops = pr[PH_HRR_OPS]; e.nint = pr[PH_NINT];
+    std::call_once(g_register_once, [] {
+        register_all_classes();
+        static const struct { int qc, la, lb, lc, ld, vrr_ops, hrr_ops, nint; } meta[] = {
+#define ADFT_CLASS_META(qc, la, lb, lc, ld, vrr_ops, hrr_ops, nint) {qc, la, lb, lc, ld, vrr_ops, hrr_ops, nint},
+#include "generated/class_meta.inc"
+#undef ADFT_CLASS_META
+        };
+        for (const auto &m : meta) {
+            ClassEntry &e = g_classes[m.qc];
+            if (e.launch_jk || !rys_jk_launcher(m.la, m.lb, m.lc, m.ld)) continue;
+            e.use_rys = true;
+            e.impl = "rys";
+            e.la = m.la; e.lb = m.lb; e.lc = m.lc; e.ld = m.ld;
+            e.vrr_ops = m.vrr_ops; e.hrr_ops = m.hrr_ops; e.nint = m.nint;
         }
-    }
-    g_registered = true;
-}
-
-static InterpProg make_prog(const ClassEntry &e, const int32_t *d_blob, bool diag)
-{
-    const int32_t *h = e.prog;
-    const int32_t *d = d_blob + e.prog_off;
-    InterpProg g{};
-    g.vrr = (const int4 *)(d + h[PH_OFF_VRR]);
-    g.hrr = (const int4 *)(d + (diag ? h[PH_OFF_DIAG] : h[PH_OFF_HRR]));
-    g.n_vrr = h[PH_NVRR];
-    g.n_hrr = diag ? h[PH_NHRR_DIAG] : h[PH_NHRR];
-    g.n_vslots = h[PH_NVSLOTS];
-    g.n_hslots = diag ? h[PH_NHSLOTS_DIAG] : h[PH_NHSLOTS];
-    g.nacc = h[PH_NACC];
-    g.mmax = h[PH_MMAX];
-    g.la = h[PH_LA]; g.lb = h[PH_LB]; g.lc = h[PH_LC]; g.ld = h[PH_LD];
-    return g;
-}
-static int jk_slots_of(const ClassEntry &e)
-{
-    const int32_t *h = e.prog;
-    return interp_jk_slots(h[PH_NVSLOTS], h[PH_NHSLOTS], h[PH_NACC], h[PH_LA], h[PH_LB], h[PH_LC], h[PH_LD]);
-}
-static int schwarz_slots_of(const ClassEntry &e)
-{
-    const int32_t *h = e.prog;
-    return h[PH_NACC] + std::max(h[PH_NVSLOTS], h[PH_NHSLOTS_DIAG]);
+    });
 }
 
 #define CUDA_TRY(expr)                                                                           \
@@ -121,13 +80,39 @@ __device__ __forceinline__ double prim_pair_estimate(double a, double b, double 
     return f;
 }
 
+// Which primitive pairs of shell pair (sa, sb) survive the primitive screen: bit ia*npb+ib of `keep` (ADFT_MAX_PRIM_PAIRS
+// bits) is set iff the estimate reaches thr; if none does, the largest one is kept.  Returns the number of set bits.
+// The count pass and the write pass of pair_prim_kernel both call THIS function (never inlined), so the two passes
+// cannot disagree on a borderline pair.
+__device__ __noinline__ int prim_keep_mask(int npa, int npb, const double *__restrict__ ea, const double *__restrict__ eb,
+                                           const double *__restrict__ ca, const double *__restrict__ cb, double AB2, int la,
+                                           int lb, double thr, uint32_t *keep)
+{
+    for (int w = 0; w < ADFT_MAX_PRIM_PAIRS / 32; ++w) keep[w] = 0u;
+    int cnt = 0, best = 0;
+    double best_est = -1.0;
+    for (int ia = 0; ia < npa; ++ia)
+        for (int ib = 0; ib < npb; ++ib) {
+            const int idx = ia * npb + ib;
+            const double est = prim_pair_estimate(ea[ia], eb[ib], ca[ia], cb[ib], AB2, la, lb);
+            if (est >= thr) { keep[idx >> 5] |= 1u << (idx & 31); ++cnt; }
+            if (est > best_est) { best_est = est; best = idx; }
+        }
+    if (cnt == 0) { keep[best >> 5] |= 1u << (best & 31); cnt = 1; }
+    return cnt;
+}
+
 // (a2) primitive-pair records of one sublist.  Two modes:
-//   kcount != NULL : count, per pair, the primitive pairs whose estimate is >= thr (at least 1: the largest is always
-//                    kept) and write the count to kcount[g]; no records are written;
-//   kcount == NULL : write the records of the surviving primitive pairs (the same rule, same arithmetic) in nominal
-//                    order (ia major, ib minor) to slots k = 0..K-1 of the sublist (all its pairs have K survivors).
-__global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int la, int lb, double thr, int32_t *kcount,
-                                 const int32_t *__restrict__ sha,
+//   kcount != NULL : write, per pair, the number of primitive pairs that survive the primitive screen to kcount[g];
+//   kcount == NULL : write the records of the surviving primitive pairs to slots k = 0..K-1 of the sublist (all its pairs
+//                    have K survivors; a pair whose count differs from K raises *err and writes nothing).
+// The survivors are stored in DESCENDING order of zeta = alpha + beta (ties: nominal order ia major, ib minor).  All
+// lanes of a warp walk primitive lists of the same length; with the lists ranked by exponent the Boys argument
+// T = rho |PQ|^2 of step (kb, kk) is large in most lanes together (tight x tight first) or small together, so the
+// T < / >= switch branches of boys_scaled are taken warp-uniformly more often.  The slot of a survivor is its rank
+// (the number of survivors that sort before it), so no per-thread sort buffer is needed.
+__global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int K, int la, int lb, double thr, int32_t *kcount,
+                                 int32_t *err, const int32_t *__restrict__ sha,
                                  const int32_t *__restrict__ shb, const int32_t *__restrict__ sh_atom,
                                  const int32_t *__restrict__ sh_nprim, const int32_t *__restrict__ sh_off,
                                  const double *__restrict__ xyz, const double *__restrict__ expo,
@@ -142,45 +127,31 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int la, in
     const double Bx = xyz[3 * sh_atom[sb]], By = xyz[3 * sh_atom[sb] + 1], Bz = xyz[3 * sh_atom[sb] + 2];
     const double AB2 = (Ax - Bx) * (Ax - Bx) + (Ay - By) * (Ay - By) + (Az - Bz) * (Az - Bz);
     const int npa = sh_nprim[sa], npb = sh_nprim[sb];
-    int cnt = 0, best = 0;
-    double best_est = -1.0;
-    for (int ia = 0; ia < npa; ++ia)
-        for (int ib = 0; ib < npb; ++ib) {
-            const double est = prim_pair_estimate(expo[sh_off[sa] + ia], expo[sh_off[sb] + ib], coef[sh_off[sa] + ia],
-                                                  coef[sh_off[sb] + ib], AB2, la, lb);
-            if (est >= thr) ++cnt;
-            if (est > best_est) { best_est = est; best = ia * npb + ib; }
-        }
-    if (kcount) { kcount[g] = cnt > 0 ? cnt : 1; return; }
+    const double *ea = expo + sh_off[sa], *eb = expo + sh_off[sb], *ca = coef + sh_off[sa], *cb = coef + sh_off[sb];
+    uint32_t keep[ADFT_MAX_PRIM_PAIRS / 32];
+    const int cnt = prim_keep_mask(npa, npb, ea, eb, ca, cb, AB2, la, lb, thr, keep);
+    if (kcount) { kcount[g] = cnt; return; }
+    if (cnt != K) { atomicExch(err, 1); return; }
     const double c0 = 5.9149671727956128778;     // sqrt(2) * pi^(5/4)
-    // The surviving primitive pairs are stored in DESCENDING order of zeta = alpha + beta (ties: nominal order).  All
-    // lanes of a warp walk primitive lists of the same length; with the lists ranked by exponent the Boys argument
-    // T = rho |PQ|^2 of step (kb, kk) is large in most lanes together (tight x tight first) or small together, so the
-    // T < / >= switch branches of boys_scaled are taken warp-uniformly more often.
-    int order[ADFT_MAX_PRIM_PAIRS];
-    double okey[ADFT_MAX_PRIM_PAIRS];
-    int nk = 0;
-    for (int ia = 0; ia < npa; ++ia)
-        for (int ib = 0; ib < npb; ++ib) {
-            const double a = expo[sh_off[sa] + ia], b = expo[sh_off[sb] + ib];
-            const bool keep = cnt > 0 ? (prim_pair_estimate(a, b, coef[sh_off[sa] + ia], coef[sh_off[sb] + ib], AB2, la, lb) >= thr)
-                                      : (ia * npb + ib == best);
-            if (!keep || nk >= ADFT_MAX_PRIM_PAIRS) continue;
-            int pos = nk++;
-            while (pos > 0 && okey[pos - 1] < a + b) { okey[pos] = okey[pos - 1]; order[pos] = order[pos - 1]; --pos; }
-            okey[pos] = a + b; order[pos] = ia * npb + ib;
+    const int np = npa * npb;
+    for (int idx = 0; idx < np; ++idx) {
+        if (!(keep[idx >> 5] >> (idx & 31) & 1u)) continue;
+        const int ia = idx / npb, ib = idx - ia * npb;
+        const double a = ea[ia], b = eb[ib];
+        const double z = a + b;
+        int k = 0;                               // rank among the survivors: larger zeta first, ties in nominal order
+        for (int o = 0; o < np; ++o) {
+            if (!(keep[o >> 5] >> (o & 31) & 1u)) continue;
+            const double zo = ea[o / npb] + eb[o % npb];
+            k += (zo > z || (zo == z && o < idx)) ? 1 : 0;
         }
-    for (int k = 0; k < nk; ++k) {
-            const int ia = order[k] / npb, ib = order[k] % npb;
-            const double a = expo[sh_off[sa] + ia], b = expo[sh_off[sb] + ib];
-            const double da = coef[sh_off[sa] + ia], db = coef[sh_off[sb] + ib];
-            const double z = a + b, iz = 1.0 / z;
-            const double px = (a * Ax + b * Bx) * iz, py = (a * Ay + b * By) * iz, pz = (a * Az + b * Bz) * iz;
-            const int idx = prim_base + k * n + j;
-            zeta[idx] = z;  inv2z[idx] = 0.5 * iz;
-            Px[idx] = px;  Py[idx] = py;  Pz[idx] = pz;
-            PAx[idx] = px - Ax;  PAy[idx] = py - Ay;  PAz[idx] = pz - Az;
-            cc[idx] = c0 * da * db * exp(-a * b * iz * AB2) * iz;
+        const double iz = 1.0 / z;
+        const double px = (a * Ax + b * Bx) * iz, py = (a * Ay + b * By) * iz, pz = (a * Az + b * Bz) * iz;
+        const int slot = prim_base + k * n + j;
+        zeta[slot] = z;  inv2z[slot] = 0.5 * iz;
+        Px[slot] = px;  Py[slot] = py;  Pz[slot] = pz;
+        PAx[slot] = px - Ax;  PAy[slot] = py - Ay;  PAz[slot] = pz - Az;
+        cc[slot] = c0 * ca[ia] * cb[ib] * exp(-a * b * iz * AB2) * iz;
     }
 }
 
@@ -248,6 +219,7 @@ struct Sublist {
 struct adft_shellpairs {
     const adft_basis *basis = nullptr;
     int64_t npairs = 0, nprimpairs = 0, nprimpairs_nominal = 0;
+    int sm_count = 148;                // of the device the table lives on
     double prim_threshold = 0.0;
     std::vector<Sublist> subl;
     std::vector<int> subl_of_class[NPAIRCLASS];
@@ -259,13 +231,13 @@ struct adft_shellpairs {
     // device: pair table
     double *d_Q = nullptr, *d_AB = nullptr /* 3*npairs */, *d_prim = nullptr /* 9*nprimpairs */;
     int32_t *d_pint = nullptr /* 5*npairs: bfa,bfb,sha,shb,knom */;
-    double *d_boys = nullptr;                 // F_m(T_k), [BOYS_NT][BOYS_NM] (interpreter)
     double *d_boysp = nullptr;                // per-order Taylor tables [BOYS_MORD][BOYS_NT][BOYS_NC] (generated kernels)
     PairTable tab{};
     // per-build workspaces
     Segment *d_segs = nullptr, *h_segs = nullptr;
     size_t segs_cap = 0;
     unsigned long long *d_counters = nullptr, *d_dmax = nullptr, *h_small = nullptr;
+    int32_t *d_prim_err = nullptr;     // raised by pair_prim_kernel when a pair's survivor count is not its sublist's K
     cudaEvent_t ev[2 * NQCLASS + 8] = {};
     bool ev_ok = false;
     // last build
@@ -276,15 +248,8 @@ struct adft_shellpairs {
     // staging for adft_jk_build_host
     double *d_stage = nullptr;
     size_t stage_n = 0;
-    // interpreter path (classes without straight-line code): device copy of the program blob, per-thread scratch
-    int32_t *d_blob = nullptr;
     double *d_rys = nullptr;                  // device copy of the Rys tables
     RysTable rys{};
-    double *d_scratch = nullptr;
-    long long scratch_threads = 0;     // threads of the persistent interpreter grid = scratch stride
-    int interp_blocks = 0;
-    // sink for the output the caller skipped (J == NULL or K == NULL): round 1 has one kernel variant per class
-    double *d_sink = nullptr;
 };
 
 // ------------------------------------------------------------------ misc API
@@ -416,8 +381,8 @@ static void free_pairs(adft_shellpairs *p)
     if (!p) return;
     cudaFree(p->d_xyz); cudaFree(p->d_expo); cudaFree(p->d_coef); cudaFree(p->d_atom); cudaFree(p->d_nprim);
     cudaFree(p->d_off); cudaFree(p->d_Q); cudaFree(p->d_AB); cudaFree(p->d_prim); cudaFree(p->d_pint);
-    cudaFree(p->d_boys); cudaFree(p->d_boysp); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage); cudaFree(p->d_sink);
-    cudaFree(p->d_blob); cudaFree(p->d_scratch); cudaFree(p->d_rys);
+    cudaFree(p->d_boysp); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage);
+    cudaFree(p->d_rys); cudaFree(p->d_prim_err);
     if (p->h_segs) cudaFreeHost(p->h_segs);
     if (p->h_small) cudaFreeHost(p->h_small);
     if (p->ev_ok) for (auto &e : p->ev) cudaEventDestroy(e);
@@ -454,18 +419,23 @@ static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vecto
     }
     CUDA_TRY(cudaMemcpyAsync(p->d_AB, AB.data(), AB.size() * sizeof(double), cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(p->d_pint, pint.data(), pint.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemsetAsync(p->d_prim_err, 0, sizeof(int32_t), st));
     CUDA_TRY(cudaStreamSynchronize(st));     // host vectors go out of scope
     const size_t npp = (size_t)p->nprimpairs;
     double *f = p->d_prim;
     for (const Sublist &s : p->subl) {
         if (s.n == 0) continue;
-        pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.la, s.lb, thr, nullptr,
-                                                             p->tab.sha, p->tab.shb, p->d_atom,
+        pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.K, s.la, s.lb, thr, nullptr,
+                                                             p->d_prim_err, p->tab.sha, p->tab.shb, p->d_atom,
                                                              p->d_nprim, p->d_off, p->d_xyz, p->d_expo, p->d_coef, f, f + npp,
                                                              f + 2 * npp, f + 3 * npp, f + 4 * npp, f + 5 * npp, f + 6 * npp,
                                                              f + 7 * npp, f + 8 * npp);
     }
     CUDA_TRY(cudaGetLastError());
+    int32_t bad = 0;
+    CUDA_TRY(cudaMemcpyAsync(&bad, p->d_prim_err, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (bad) { set_error("adft_shellpairs_build: primitive-pair count of a pair differs from its sublist's depth"); return ADFT_ERR_INTERNAL; }
     return ADFT_OK;
 }
 
@@ -519,6 +489,11 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     adft_shellpairs *p = new (std::nothrow) adft_shellpairs;
     if (!p) return ADFT_ERR_ALLOC;
     p->basis = b;
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+            p->sm_count = sms;
+    }
     const int ns = b->nshells;
 
     p->prim_threshold = prim_threshold;
@@ -553,7 +528,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     // every needed Schwarz class must exist
     for (const Sublist &s : p->subl) {
         const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
-        if (!ce.launch_schwarz && !ce.prog) {
+        if (!ce.launch_schwarz && !(ce.use_rys && rys_schwarz_launcher(s.la, s.lb))) {
             set_error("adft_shellpairs_build: no kernel for pair class (" + std::to_string(s.la) + "," + std::to_string(s.lb) + ")");
             free_pairs(p); return ADFT_ERR_UNSUPPORTED_L;
         }
@@ -575,30 +550,10 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     ALLOC(p->d_AB, 3 * np * sizeof(double));
     ALLOC(p->d_pint, 5 * np * sizeof(int32_t));
     ALLOC(p->d_prim, 9 * npp * sizeof(double));
-    ALLOC(p->d_boys, (size_t)BOYS_NT * BOYS_NM * sizeof(double));
     ALLOC(p->d_boysp, (size_t)BOYS_MORD * BOYS_NT * BOYS_NC * sizeof(double));
     ALLOC(p->d_counters, 4 * NQCLASS * sizeof(unsigned long long));
-    {
-        // interpreter resources, only if some class that can occur lacks straight-line code
-        int slots = 0;
-        for (int X = 0; X < NPAIRCLASS; ++X)
-            for (int Y = 0; Y <= X; ++Y) {
-                if (p->subl_of_class[X].empty() || p->subl_of_class[Y].empty()) continue;
-                const ClassEntry &ce = class_table()[quartet_class(X, Y)];
-                if (ce.use_table) slots = std::max(slots, jk_slots_of(ce));
-                if (X == Y && (ce.use_table || (!ce.launch_schwarz && !ce.use_rys))) slots = std::max(slots, schwarz_slots_of(ce));
-            }
-        if (slots > 0) {
-            int dev = 0, sms = 0;
-            cudaGetDevice(&dev);
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            p->interp_blocks = sms * 4;
-            p->scratch_threads = (long long)p->interp_blocks * 128;
-            ALLOC(p->d_blob, (size_t)(adft_prog_blob_end - adft_prog_blob) * sizeof(int32_t));
-            ALLOC(p->d_scratch, (size_t)slots * (size_t)p->scratch_threads * sizeof(double));
-        }
-    }
     ALLOC(p->d_dmax, 2 * sizeof(unsigned long long));
+    ALLOC(p->d_prim_err, sizeof(int32_t));
     ALLOC(p->d_rys, (size_t)(adft_rys_blob_end - adft_rys_blob) * sizeof(double));
 #undef ALLOC
     {
@@ -639,12 +594,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     TRY2(cudaMemcpyAsync(p->d_off, b->off.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     TRY2(cudaMemcpyAsync(p->d_rys, adft_rys_blob, (size_t)(adft_rys_blob_end - adft_rys_blob) * sizeof(double),
                          cudaMemcpyHostToDevice, st));
-    if (p->d_blob)
-        TRY2(cudaMemcpyAsync(p->d_blob, adft_prog_blob, (size_t)(adft_prog_blob_end - adft_prog_blob) * sizeof(int32_t),
-                             cudaMemcpyHostToDevice, st));
     std::vector<double> boys;
     fill_boys_table(boys);
-    TRY2(cudaMemcpyAsync(p->d_boys, boys.data(), boys.size() * sizeof(double), cudaMemcpyHostToDevice, st));
     // per-order tables: a_j = F_{M+j}(T_k) / j!, j = 0..9  (Taylor coefficients of F_M about T_k in d = T_k - T)
     std::vector<double> boysp((size_t)BOYS_MORD * BOYS_NT * BOYS_NC);
     for (int M = 0; M < BOYS_MORD; ++M)
@@ -664,18 +615,10 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     for (const Sublist &s : p->subl) {
         if (s.n == 0) continue;
         const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
-        if (ce.launch_schwarz && !ce.use_table) {
+        if (ce.launch_schwarz) {
             ce.launch_schwarz(p->tab, s.pair_base, s.prim_base, s.n, s.K, p->d_boysp, p->d_Q, st);
-        } else if (ce.use_rys && rys_schwarz_launcher(s.la, s.lb)) {
-            TRY2(rys_schwarz_launcher(s.la, s.lb)(p->tab, p->rys, s.pair_base, s.prim_base, s.n, s.K, p->d_Q, st));
         } else {
-            const InterpProg pg = make_prog(ce, p->d_blob, true);
-            for (long long first = 0; first < s.n; first += p->scratch_threads) {
-                const int count = (int)std::min<long long>(p->scratch_threads, s.n - first);
-                schwarz_interp_kernel<<<(count + 127) / 128, 128, 0, st>>>(p->tab, pg, s.pair_base, s.prim_base, s.n, s.K,
-                                                                          (int)first, count, p->d_boys, p->d_Q,
-                                                                          p->d_scratch, p->scratch_threads);
-            }
+            TRY2(rys_schwarz_launcher(s.la, s.lb)(p->tab, p->rys, s.pair_base, s.prim_base, s.n, s.K, p->d_Q, st));
         }
     }
     TRY2(cudaGetLastError());
@@ -691,8 +634,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
         int32_t *d_kcount = p->d_pint + 4 * np;          // the knom slot is rewritten in pass 2
         for (const Sublist &s : p->subl) {
             if (s.n == 0) continue;
-            pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.la, s.lb, prim_threshold,
-                                                                 d_kcount, p->tab.sha, p->tab.shb, p->d_atom, p->d_nprim,
+            pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.K, s.la, s.lb, prim_threshold,
+                                                                 d_kcount, p->d_prim_err, p->tab.sha, p->tab.shb, p->d_atom, p->d_nprim,
                                                                  p->d_off, p->d_xyz, p->d_expo, p->d_coef, nullptr, nullptr,
                                                                  nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
         }
@@ -804,7 +747,7 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
 {
     if (!p || !D || (!J && !K)) { set_error("adft_jk_build: NULL handle or D, or both J and K NULL"); return ADFT_ERR_INVALID_ARG; }
     if (!(tau >= 0.0) || !std::isfinite(tau)) { set_error("adft_jk_build: schwarz_threshold must be finite and >= 0"); return ADFT_ERR_INVALID_ARG; }
-    if (D == J || D == K) { set_error("adft_jk_build: D must not alias J or K"); return ADFT_ERR_INVALID_ARG; }
+    if (D == J || D == K || J == K) { set_error("adft_jk_build: D, J and K must not alias one another"); return ADFT_ERR_INVALID_ARG; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int N = p->basis->nbf;
     const size_t n2 = (size_t)N * N;
@@ -813,19 +756,17 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
     for (int X = 0; X < NPAIRCLASS; ++X)
         for (int Y = 0; Y <= X; ++Y)
             if (!p->subl_of_class[X].empty() && !p->subl_of_class[Y].empty() && !class_table()[quartet_class(X, Y)].launch_jk &&
-                !class_table()[quartet_class(X, Y)].use_table && !class_table()[quartet_class(X, Y)].use_rys) {
+                !class_table()[quartet_class(X, Y)].use_rys) {
                 set_error("adft_jk_build: no kernel compiled for quartet class " + std::to_string(quartet_class(X, Y)));
                 return ADFT_ERR_UNSUPPORTED_L;
             }
-    if ((!J || !K) && !p->d_sink) CUDA_TRY(cudaMalloc((void **)&p->d_sink, n2 * sizeof(double)));
-    double *Jw = J ? J : p->d_sink, *Kw = K ? K : p->d_sink;
     cudaEvent_t *ev = p->ev;
     cudaEvent_t ev_begin = ev[2 * NQCLASS], ev_dmax = ev[2 * NQCLASS + 1], ev_plan = ev[2 * NQCLASS + 2],
                 ev_eri = ev[2 * NQCLASS + 3], ev_end = ev[2 * NQCLASS + 4];
     CUDA_TRY(cudaEventRecord(ev_begin, st));
     // (a3) Dmax
     CUDA_TRY(cudaMemsetAsync(p->d_dmax, 0, 2 * sizeof(unsigned long long), st));
-    dmax_kernel<<<592, 256, 0, st>>>(D, n2, p->d_dmax); ++launches;
+    dmax_kernel<<<(unsigned)std::min<size_t>((n2 + 255) / 256, (size_t)p->sm_count * 4), 256, 0, st>>>(D, n2, p->d_dmax); ++launches;
     CUDA_TRY(cudaMemcpyAsync(p->h_small, p->d_dmax, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaEventRecord(ev_dmax, st));
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -876,20 +817,12 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         if (warps[qc] == 0) continue;
         JKParams prm{};
         prm.t = p->tab; prm.segs = p->d_segs + seg_off[qc]; prm.nsegs = (int)plan[qc].size(); prm.total_warps = warps[qc];
-        prm.D = D; prm.J = Jw; prm.K = Kw; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boysp;
+        prm.D = D; prm.J = J; prm.K = K; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boysp;
         prm.counters = p->d_counters + 4 * qc; prm.zero = 0;
         CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
         const ClassEntry &ce = class_table()[qc];
         if (ce.use_rys) {
-            CUDA_TRY(rys_jk_launcher(ce.la, ce.lb, ce.lc, ce.ld)(prm, p->rys, p->d_counters + 4 * qc + 3, st));
-        } else if (ce.use_table) {
-            InterpParams ip{};
-            ip.jk = prm; ip.prog = make_prog(ce, p->d_blob, false);
-            ip.scratch = p->d_scratch; ip.stride = p->scratch_threads;
-            ip.tile_counter = p->d_counters + 4 * qc + 3;
-            ip.boys_plain = p->d_boys;
-            const long long want = (warps[qc] + 3) / 4;
-            jk_interp_kernel<<<(unsigned)std::min<long long>(want, p->interp_blocks), 128, 0, st>>>(ip);
+            CUDA_TRY(rys_jk_launcher(ce.la, ce.lb, ce.lc, ce.ld)(prm, p->rys, p->d_counters + 4 * qc + 3, st, J != nullptr, K != nullptr));
         } else {
             ce.launch_jk(prm, st, J != nullptr, K != nullptr);
         }

@@ -1,24 +1,48 @@
 // adft_rys.cu -- instantiations of the block-cooperative Rys kernels (adft_rys.cuh) for the quartet classes without
 // straight-line code, and of the Schwarz kernels of the pair classes (fp), (fd), (ff).
+#include <atomic>
+
 #include "adft_internal.h"
 #include "adft_rys.cuh"
 
 namespace adft {
 
-template <class C>
-static cudaError_t run_jk(const JKParams &p, const RysTable &rt, unsigned long long *tile_counter, cudaStream_t st)
+// resident blocks of the persistent grid, per device (occupancy x SM count), computed once per device
+template <class C, bool WJ, bool WK>
+static int resident_blocks()
 {
-    static int nblocks = 0;
-    if (nblocks == 0) {
-        int dev = 0, sms = 0, occ = 0;
-        cudaGetDevice(&dev);
+    constexpr int MAXDEV = 64;
+    static std::atomic<int> cache[MAXDEV];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= MAXDEV) dev = 0;
+    int nb = cache[dev].load(std::memory_order_relaxed);
+    if (nb == 0) {
+        int sms = 0, occ = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(jk_rys_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jk_rys_kernel<C>, C::NT, C::SMEM_BYTES);
-        nblocks = sms * (occ > 0 ? occ : 1);
+        cudaFuncSetAttribute(jk_rys_kernel<C, WJ, WK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jk_rys_kernel<C, WJ, WK>, C::NT, C::SMEM_BYTES);
+        nb = sms * (occ > 0 ? occ : 1);
+        cache[dev].store(nb, std::memory_order_relaxed);
     }
+    return nb;
+}
+
+template <class C, bool WJ, bool WK>
+static cudaError_t run_jk_variant(const JKParams &p, const RysTable &rt, unsigned long long *tile_counter, cudaStream_t st)
+{
+    const int nblocks = resident_blocks<C, WJ, WK>();
     const long long want = p.total_warps;
-    return launch_jk_rys<C>(p, rt, tile_counter, (int)(want < nblocks ? want : nblocks), st);
+    return launch_jk_rys<C, WJ, WK>(p, rt, tile_counter, (int)(want < nblocks ? want : nblocks), st);
+}
+
+template <class C>
+static cudaError_t run_jk(const JKParams &p, const RysTable &rt, unsigned long long *tile_counter, cudaStream_t st,
+                          bool want_j, bool want_k)
+{
+    if (want_j && want_k) return run_jk_variant<C, true, true>(p, rt, tile_counter, st);
+    if (want_j) return run_jk_variant<C, true, false>(p, rt, tile_counter, st);
+    return run_jk_variant<C, false, true>(p, rt, tile_counter, st);
 }
 
 template <class C>

@@ -269,8 +269,9 @@ __device__ __forceinline__ void rys_phase2_dispatch(int chunk, const double *__r
     else if constexpr (CHK + 1 < C::NCH) rys_phase2_dispatch<C, CHK + 1>(chunk, sm, nb, offx, offy, offz, acc);
 }
 
-// (a5) digestion of the integrals a thread owns: (ia ib | q), q = CHK*CH + n.  Same six updates as DigestJK.
-template <class C, int CHK>
+// (a5) digestion of the integrals a thread owns: (ia ib | q), q = CHK*CH + n.  Same six updates as DigestJK; WJ / WK
+// select the J-only and K-only instantiations (the skipped matrix costs no loads, FMAs or reductions).
+template <class C, int CHK, bool WJ, bool WK>
 struct RysDigest {
     double jab, kac[C::NC], kad[C::ND], kbc[C::NC], kbd[C::ND];
     const double *D;
@@ -285,17 +286,21 @@ struct RysDigest {
         if constexpr (q < C::NCD) {
             constexpr int ic = q / C::ND, id = q % C::ND;
             const double v = acc[n];
-            jab = fma(__ldg(D + (size_t)(c0 + ic) * N + d0 + id), v, jab);
-            double t = dab2 * v;                                        // J_cd: the lanes of a warp share (ic, id)
+            if constexpr (WJ) {
+                jab = fma(__ldg(D + (size_t)(c0 + ic) * N + d0 + id), v, jab);
+                double t = dab2 * v;                                        // J_cd: the lanes of a warp share (ic, id)
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-            if (lane == 0) atomicAdd(J + (size_t)(c0 + ic) * N + d0 + id, t);
-            const double Dbd = __ldg(D + (size_t)rb * N + d0 + id), Dbc = __ldg(D + (size_t)rb * N + c0 + ic);
-            const double Dad = __ldg(D + (size_t)ra * N + d0 + id), Dac = __ldg(D + (size_t)ra * N + c0 + ic);
-            kac[ic] = fma(Dbd, v, kac[ic]);
-            kad[id] = fma(Dbc, v, kad[id]);
-            kbc[ic] = fma(Dad, v, kbc[ic]);
-            kbd[id] = fma(Dac, v, kbd[id]);
+                for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                if (lane == 0) atomicAdd(J + (size_t)(c0 + ic) * N + d0 + id, t);
+            }
+            if constexpr (WK) {
+                const double Dbd = __ldg(D + (size_t)rb * N + d0 + id), Dbc = __ldg(D + (size_t)rb * N + c0 + ic);
+                const double Dad = __ldg(D + (size_t)ra * N + d0 + id), Dac = __ldg(D + (size_t)ra * N + c0 + ic);
+                kac[ic] = fma(Dbd, v, kac[ic]);
+                kad[id] = fma(Dbc, v, kad[id]);
+                kbc[ic] = fma(Dad, v, kbc[ic]);
+                kbd[id] = fma(Dac, v, kbd[id]);
+            }
         }
     }
     template <int... Ns>
@@ -337,7 +342,7 @@ struct RysDigest {
     {
         D = p.D; J = p.J; N = p.N; ra = a0 + ia; rb = b0 + ib; c0 = c0_; d0 = d0_; lane = lane_;
         const double w = active ? wgt : 0.0;
-        dab2 = (w + w) * __ldg(D + (size_t)ra * N + rb);
+        dab2 = WJ ? (w + w) * __ldg(D + (size_t)ra * N + rb) : 0.0;
         jab = 0.0;
 #pragma unroll
         for (int x = 0; x < C::NC; ++x) kac[x] = kbc[x] = 0.0;
@@ -345,18 +350,20 @@ struct RysDigest {
         for (int x = 0; x < C::ND; ++x) kad[x] = kbd[x] = 0.0;
         all(acc, std::make_integer_sequence<int, C::CH>{});
         if (active) {
-            atomicAdd(J + (size_t)ra * N + rb, (w + w) * jab);
-            flush_cs(p.K, w, std::make_integer_sequence<int, C::NC>{});
-            flush_ds(p.K, w, std::make_integer_sequence<int, C::ND>{});
+            if constexpr (WJ) atomicAdd(J + (size_t)ra * N + rb, (w + w) * jab);
+            if constexpr (WK) {
+                flush_cs(p.K, w, std::make_integer_sequence<int, C::NC>{});
+                flush_ds(p.K, w, std::make_integer_sequence<int, C::ND>{});
+            }
         }
     }
 };
-template <class C, int CHK = 0>
+template <class C, bool WJ, bool WK, int CHK = 0>
 __device__ __forceinline__ void rys_digest_dispatch(int chunk, const double (&acc)[C::CH], bool active, int ia, int ib,
                                                     const JKParams &p, int a0, int b0, int c0, int d0, double wgt, int lane)
 {
-    if (chunk == CHK) { RysDigest<C, CHK> dg; dg.run(acc, active, ia, ib, p, a0, b0, c0, d0, wgt, lane); }
-    else if constexpr (CHK + 1 < C::NCH) rys_digest_dispatch<C, CHK + 1>(chunk, acc, active, ia, ib, p, a0, b0, c0, d0, wgt, lane);
+    if (chunk == CHK) { RysDigest<C, CHK, WJ, WK> dg; dg.run(acc, active, ia, ib, p, a0, b0, c0, d0, wgt, lane); }
+    else if constexpr (CHK + 1 < C::NCH) rys_digest_dispatch<C, WJ, WK, CHK + 1>(chunk, acc, active, ia, ib, p, a0, b0, c0, d0, wgt, lane);
 }
 
 // contracted integrals of one shell quartet into the registers of the block (both phases, all batches)
@@ -386,7 +393,7 @@ __device__ __forceinline__ void rys_quartet(const PairTable &t, const RysTable &
     }
 }
 
-template <class C>
+template <class C, bool WJ, bool WK>
 __global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p, const RysTable rt, unsigned long long *tile_counter)
 {
     extern __shared__ double sm[];
@@ -436,7 +443,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p
             if (sa == sb) wgt *= 0.5;
             if (sc == sd) wgt *= 0.5;
             if (gab == gcd) wgt *= 0.5;
-            rys_digest_dispatch<C>(chunk, acc, active, ia, ib, p, a0, b0, __ldg(p.t.bfa + gcd), __ldg(p.t.bfb + gcd), wgt, lane);
+            rys_digest_dispatch<C, WJ, WK>(chunk, acc, active, ia, ib, p, a0, b0, __ldg(p.t.bfa + gcd), __ldg(p.t.bfb + gcd), wgt, lane);
         }
     }
     if (tid == 0 && cnt_q) {
@@ -489,10 +496,10 @@ __global__ void __launch_bounds__(C::NT, 1) schwarz_rys_kernel(const PairTable t
     }
 }
 
-template <class C>
+template <class C, bool WJ, bool WK>
 inline cudaError_t launch_jk_rys(const JKParams &p, const RysTable &rt, unsigned long long *tile_counter, int nblocks, cudaStream_t st)
 {
-    auto kern = jk_rys_kernel<C>;
+    auto kern = jk_rys_kernel<C, WJ, WK>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(tile_counter, 0, sizeof(unsigned long long), st);

@@ -449,6 +449,15 @@ def main():
         metas.append(meta)
     with open(os.path.join(args.out, "classes.json"), "w") as f:
         json.dump(metas, f, indent=1)
+    # angular momenta and FP64 instruction counts of ALL classes (also those that run through the Rys kernels):
+    # the library's class table and its model-flop count read this list
+    with open(os.path.join(args.out, "class_meta.inc"), "w") as f:
+        f.write("// GENERATED: ADFT_CLASS_META(qc, la, lb, lc, ld, vrr_ops, hrr_ops, nint)\n")
+        for (la, lb, lc, ld) in all_classes(3):
+            X, Y = la * (la + 1) // 2 + lb, lc * (lc + 1) // 2 + ld
+            v, h = best_vrr(la, lb, lc, ld), HrrDag(la, lb, lc, ld)
+            f.write(f"ADFT_CLASS_META({X * (X + 1) // 2 + Y}, {la}, {lb}, {lc}, {ld}, {v.fp64_ops()}, {h.fp64_ops()}, "
+                    f"{ncart(la) * ncart(lb) * ncart(lc) * ncart(ld)})\n")
     # X-macro list of straight-line classes
     with open(os.path.join(args.out, "classes.inc"), "w") as f:
         f.write("// GENERATED: ADFT_GEN_CLASS(la, lb, lc, ld, tag)\n")
@@ -456,243 +465,6 @@ def main():
             la, lb, lc, ld = m["l"]
             f.write(f"ADFT_GEN_CLASS({la}, {lb}, {lc}, {ld}, {m['tag']})\n")
     print(f"generated {len(metas)} classes into {args.out}")
-
-
-# ----------------------------------------------------------------------------------------------------------------
-# Table programs for the interpreter kernels (classes too large for straight-line code: everything with an f shell).
-# The same DAGs as above are serialised as int32 instruction lists; value slots are assigned by liveness (linear scan)
-# so that the per-thread scratch stays small.  Layout (little-endian int32):
-#   header[32]: magic 0x41444654, la, lb, lc, ld, n_vrr, n_vslots, nacc, n_hrr, n_hslots, n_out, mmax, vrr_ops, hrr_ops,
-#               nint, n_hrr_diag, n_hslots_diag, n_out_diag, off_vrr, off_hrr, off_hrr_diag, total_len, 0...
-#               (offsets and lengths in int32 units from the start of the program)
-#   vrr[n_vrr][8]:  kind | dir<<4, dst, s0, s1, s2, s3, n2, nx      kind: 0 B (s0 = m), 1 T(bra), 2 T(ket), 3 A, 4 K,
-#                   5 ACC (acc[n2] += v[s0]);  unused operands are -1
-#   hrr[n_hrr][4]:  which | dir<<2 (which: 0 AB, 1 CD), dst, k0, k1  with h[dst] = v(k0) + G_dir * v(k1);
-#                   operands >= 0 are h slots, operands < 0 are accumulators -(1+index);
-#                   which = 2 is an OUTPUT record: dst = ia | ib<<8 | ic<<16 | id<<24, k0 = the integral's operand
-#                   (outputs are interleaved with the recurrences in execution order; n_hrr counts both)
-#   hrr_diag:       the same for the diagonal integrals (mu nu|mu nu) of classes (ab|ab) (Schwarz bound)
-#   every list is followed by one all-zero pad instruction (the interpreter prefetches one ahead)
-import struct
-
-K_B, K_TBRA, K_TKET, K_A, K_K, K_ACC = 0, 1, 2, 3, 4, 5
-
-
-def _alloc_slots(order, uses):
-    """order: list of keys that need a slot, in execution order; uses[i]: keys read at step i.  Returns (slot, n)."""
-    last = {}
-    for i, us in enumerate(uses):
-        for u in us:
-            last[u] = i
-    dying = {}
-    for k, i in last.items():
-        dying.setdefault(i, []).append(k)
-    free, slot, n = [], {}, 0
-    for i, k in enumerate(order):
-        if k is not None:
-            if free:
-                slot[k] = free.pop()
-            else:
-                slot[k] = n; n += 1
-            if k not in last:              # never read (cannot happen for pruned DAGs, kept for safety)
-                free.append(slot[k])
-        for d in dying.get(i, []):
-            free.append(slot[d])
-    return slot, n
-
-
-def vrr_program(dag):
-    tgt = {("V", a, c, 0): j for j, (a, c) in enumerate(dag.targets)}
-    steps = []            # (key or None, spec)
-    for key, s in dag.nodes.items():
-        steps.append((key, s))
-        if key in tgt:
-            steps.append((None, ("ACC", key, tgt[key])))
-    order = [k for k, _ in steps]
-    uses = []
-    for k, s in steps:
-        if s[0] == "B":
-            uses.append([])
-        elif s[0] == "T":
-            uses.append([s[2], s[3]])
-        elif s[0] == "A":
-            uses.append([x for x in (s[2], s[3], s[5]) if x])
-        elif s[0] == "K":
-            uses.append([x for x in (s[2], s[3], s[5], s[7]) if x])
-        else:
-            uses.append([s[1]])
-    slot, n = _alloc_slots(order, uses)
-    g = lambda k: slot[k] if k else -1
-    ins = []
-    for k, s in steps:
-        if s[0] == "B":
-            ins += [K_B, slot[k], s[1], -1, -1, -1, 0, 0]
-        elif s[0] == "T":
-            ins += [K_TBRA if s[1] == "bra" else K_TKET, slot[k], g(s[2]), g(s[3]), -1, -1, 0, 0]
-        elif s[0] == "A":
-            ins += [K_A | (s[1] << 4), slot[k], g(s[2]), g(s[3]), g(s[5]), -1, s[4], 0]
-        elif s[0] == "K":
-            ins += [K_K | (s[1] << 4), slot[k], g(s[2]), g(s[3]), g(s[5]), g(s[7]), s[4], s[6]]
-        else:
-            ins += [K_ACC, -1, slot[s[1]], -1, -1, -1, s[2], 0]
-    return ins, len(steps), n
-
-
-def hrr_program(hdag):
-    def resolve(k):
-        s = hdag.nodes[k]
-        while s[0] == "alias":
-            k = s[1]; s = hdag.nodes[k]
-        return k
-    steps, seen = [], set()
-
-    def visit(k):
-        k = resolve(k)
-        if k in seen:
-            return
-        seen.add(k)
-        s = hdag.nodes[k]
-        if s[0] == "acc":
-            return
-        visit(s[3]); visit(s[4])
-        steps.append(("h", k))
-    outs = []
-    for (ia, ib, ic, idd, k) in hdag.outputs:
-        visit(k)
-        steps.append(("o", (ia, ib, ic, idd, resolve(k))))
-    order, uses = [], []
-    for t, x in steps:
-        if t == "h":
-            s = hdag.nodes[x]
-            order.append(x)
-            uses.append([y for y in (resolve(s[3]), resolve(s[4])) if hdag.nodes[y][0] != "acc"])
-        else:
-            order.append(None)
-            uses.append([x[4]] if hdag.nodes[x[4]][0] != "acc" else [])
-    slot, n = _alloc_slots(order, uses)
-
-    def enc(k):
-        s = hdag.nodes[k]
-        return -(1 + s[1]) if s[0] == "acc" else slot[k]
-    ins, out = [], []
-    # outputs are interleaved with the recurrences in execution order: an output record is an hrr instruction with
-    # which = 2 and (dst, k0, k1) = (packed component indices, src, 0)
-    for t, x in steps:
-        if t == "h":
-            s = hdag.nodes[x]
-            ins += [(0 if s[1] == "AB" else 1) | (s[2] << 2), slot[x], enc(resolve(s[3])), enc(resolve(s[4]))]
-        else:
-            ia, ib, ic, idd, k = x
-            ins += [2, ia | (ib << 8) | (ic << 16) | (idd << 24), enc(k), 0]
-    return ins, len(steps), n, sum(1 for t, _ in steps if t == "o")
-
-
-def pack_program(la, lb, lc, ld):
-    """int32 list of one class program (layout above) plus its meta dict."""
-    vrr = best_vrr(la, lb, lc, ld)
-    hrr = HrrDag(la, lb, lc, ld)
-    vins, nv, nvs = vrr_program(vrr)
-    hins, nh, nhs, nout = hrr_program(hrr)
-    if (la, lb) == (lc, ld):
-        dins, ndh, ndhs, ndout = hrr_program(HrrDag(la, lb, lc, ld, diag_only=True))
-    else:
-        dins, ndh, ndhs, ndout = [], 0, 0, 0
-    nint = ncart(la) * ncart(lb) * ncart(lc) * ncart(ld)
-    # every list is padded by one all-zero instruction: the interpreter prefetches instruction i+1 while executing i
-    vins = vins + [0] * 8
-    hins = hins + [0] * 4
-    dins = dins + [0] * 4
-    off_v = 32
-    off_h = off_v + len(vins)
-    off_d = off_h + len(hins)
-    total = off_d + len(dins)
-    header = [0x41444654, la, lb, lc, ld, nv, nvs, len(vrr.targets), nh, nhs, nout, vrr.max_m(), vrr.fp64_ops(),
-              hrr.fp64_ops(), nint, ndh, ndhs, ndout, off_v, off_h, off_d, total]
-    header += [0] * (32 - len(header))
-    meta = {"tag": class_tag(la, lb, lc, ld), "l": [la, lb, lc, ld], "vrr_ops": vrr.fp64_ops(), "hrr_ops": hrr.fp64_ops(),
-            "nint": nint, "nacc": len(vrr.targets), "n_vrr": nv, "n_vslots": nvs, "n_hrr": nh, "n_hslots": nhs,
-            "how": vrr.how}
-    return header + vins + hins + dins, meta
-
-
-def write_program(path, la, lb, lc, ld):
-    data, meta = pack_program(la, lb, lc, ld)
-    with open(path, "wb") as f:
-        f.write(struct.pack("<%di" % len(data), *data))
-    return meta
-
-
-def write_blob(path, classes):
-    """All class programs in one file: int32 dir[56][2] = (offset, length) in int32 units indexed by quartet class
-    qc = X(X+1)/2+Y (X >= Y pair classes, pc = la(la+1)/2+lb), zero if absent; then the programs (16-byte aligned)."""
-    ndir = 56
-    directory = [0] * (2 * ndir)
-    body, metas = [], []
-    for (la, lb, lc, ld) in classes:
-        data, meta = pack_program(la, lb, lc, ld)
-        X, Y = la * (la + 1) // 2 + lb, lc * (lc + 1) // 2 + ld
-        qc = X * (X + 1) // 2 + Y
-        assert len(data) % 4 == 0
-        directory[2 * qc] = 2 * ndir + len(body)
-        directory[2 * qc + 1] = len(data)
-        body += data
-        metas.append(meta)
-    data = directory + body
-    with open(path, "wb") as f:
-        f.write(struct.pack("<%di" % len(data), *data))
-    return metas
-
-
-def eval_program(path, ctx, AB, CD, diag=False):
-    """Python interpreter of a program file (mirror of the CUDA interpreter) -- used by tests/test_codegen.py."""
-    raw = open(path, "rb").read()
-    d = struct.unpack("<%di" % (len(raw) // 4), raw)
-    assert d[0] == 0x41444654
-    la, lb, lc, ld, nv, nvs, nacc, nh, nhs, nout, mmax = d[1:12]
-    ndh, ndhs, ndout = d[15:18]
-    off_v, off_h, off_d, total = d[18:22]
-    assert total == len(d)
-    v = [0.0] * max(nvs, 1)
-    acc = [0.0] * nacc
-    p = off_v
-    for i in range(nv):
-        op, dst, s0, s1, s2, s3, n2, nx = d[p:p + 8]; p += 8
-        kind, dr = op & 15, (op >> 4) & 3
-        if kind == K_B:
-            v[dst] = ctx["F"][s0]
-        elif kind == K_TBRA:
-            v[dst] = v[s0] - ctx["roz"] * v[s1]
-        elif kind == K_TKET:
-            v[dst] = v[s0] - ctx["roe"] * v[s1]
-        elif kind == K_A:
-            x = ctx["PA"][dr] * v[s0] + ctx["WP"][dr] * v[s1]
-            if s2 >= 0:
-                x += n2 * ctx["inv2z"] * v[s2]
-            v[dst] = x
-        elif kind == K_K:
-            x = ctx["QC"][dr] * v[s0] + ctx["WQ"][dr] * v[s1]
-            if s2 >= 0:
-                x += n2 * ctx["inv2e"] * v[s2]
-            if s3 >= 0:
-                x += nx * ctx["inv2ze"] * v[s3]
-            v[dst] = x
-        else:
-            acc[n2] += v[s0]
-    p = off_h
-    if diag:
-        p = off_d
-        nh, nhs = ndh, ndhs
-    h = [0.0] * max(nhs, 1)
-    rd = lambda k: acc[-k - 1] if k < 0 else h[k]
-    out = {}
-    for i in range(nh):
-        op, dst, k0, k1 = d[p:p + 4]; p += 4
-        which, dr = op & 3, (op >> 2) & 3
-        if which == 2:
-            out[(dst & 255, (dst >> 8) & 255, (dst >> 16) & 255, (dst >> 24) & 255)] = rd(k0)
-        else:
-            h[dst] = rd(k0) + (AB if which == 0 else CD)[dr] * rd(k1)
-    return out
 
 
 if __name__ == "__main__":

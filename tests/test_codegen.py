@@ -61,44 +61,3 @@ def test_all_direction_rules_agree():
         acc = np.array(gen_eri.VrrDag(2, 1, 2, 1, how).evaluate(ctx))
         base = acc if base is None else base
         np.testing.assert_allclose(acc, base, rtol=1e-12, atol=1e-14)
-
-
-@pytest.mark.parametrize("cls", [(1, 0, 0, 0), (2, 1, 1, 1), (2, 2, 2, 2), (3, 1, 2, 0), (3, 2, 3, 2), (3, 3, 3, 3)],
-                         ids=lambda c: "".join("spdf"[x] for x in c))
-def test_table_program_matches_dag(tmp_path, cls):
-    """The serialised table program (what the CUDA interpreter executes), run by its Python mirror, reproduces the
-    DAG evaluation exactly, including the diagonal-only program of classes (ab|ab)."""
-    la, lb, lc, ld = cls
-    rng = np.random.default_rng(11 + sum(cls))
-    cen = rng.normal(0, 0.9, size=(4, 3))
-    z = np.exp(rng.uniform(np.log(0.3), np.log(4.0), size=4))
-    ctx = prim_ctx(*z, *cen, la + lb + lc + ld)
-    path = str(tmp_path / "p.bin")
-    meta = gen_eri.write_program(path, la, lb, lc, ld)
-    AB, CD = cen[0] - cen[1], cen[2] - cen[3]
-    got = gen_eri.eval_program(path, ctx, AB, CD)
-    acc = gen_eri.best_vrr(la, lb, lc, ld).evaluate(ctx)
-    ref = gen_eri.HrrDag(la, lb, lc, ld).evaluate(acc, AB, CD)
-    assert got.keys() == ref.keys() and len(got) == meta["nint"]
-    for k in ref:
-        assert abs(got[k] - ref[k]) <= 1e-13 * max(1.0, abs(ref[k]))
-    if (la, lb) == (lc, ld):
-        dg = gen_eri.eval_program(path, ctx, AB, CD, diag=True)
-        rd = gen_eri.HrrDag(la, lb, lc, ld, diag_only=True).evaluate(acc, AB, CD)
-        assert dg.keys() == rd.keys()
-        for k in rd:
-            assert abs(dg[k] - rd[k]) <= 1e-13 * max(1.0, abs(rd[k]))
-
-
-def test_blob_directory(tmp_path):
-    import struct
-    path = str(tmp_path / "blob.bin")
-    classes = [(0, 0, 0, 0), (2, 1, 1, 0), (3, 0, 3, 0)]
-    gen_eri.write_blob(path, classes)
-    raw = open(path, "rb").read()
-    d = struct.unpack("<%di" % (len(raw) // 4), raw)
-    for (la, lb, lc, ld) in classes:
-        X, Y = la * (la + 1) // 2 + lb, lc * (lc + 1) // 2 + ld
-        off, ln = d[2 * (X * (X + 1) // 2 + Y)], d[2 * (X * (X + 1) // 2 + Y) + 1]
-        assert off % 4 == 0 and ln > 32 and d[off] == 0x41444654 and list(d[off + 1:off + 5]) == [la, lb, lc, ld]
-        assert d[off + 21] == ln

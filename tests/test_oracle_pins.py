@@ -349,7 +349,9 @@ def test_p15_recurrence_centre_order_independence(orc, ls):
     must hold to rounding whichever order the shells are handed over in -- also in plain fp64, also for the case that
     broke the single-orientation core: a very tight high-l shell 11 bohr from a shell with a diffuse primitive
     (cfg 3 shells (242, 294): relative error 33% on Q in long double before R-22).  A wrong index permutation when the
-    four orientation groups are added, or a primitive pair counted in two groups or in none, fails this test."""
+    four orientation groups are added, or a primitive pair left out of every group, fails this test.  (A tie alpha == beta
+    counted in BOTH groups is order-symmetric and would pass here: that mistake is caught by P5, whose two shells carry
+    the same exponent set and whose golden values a double-counted tie changes, and by P16's mpmath values.)"""
     atoms = np.array([[0.0, 0.0, 0.0], [6.3, -7.1, 5.4], [0.4, 1.1, -0.3], [5.9, -6.5, 5.0]])
     la, lb = ls
     exps = {0: [4595.251], 1: [38.639, 0.05, 376.079], 2: [2019.87, 0.246, 4.992], 3: [1.7, 0.3]}
@@ -378,3 +380,27 @@ def test_p15_recurrence_centre_order_independence(orc, ls):
     for (A, B) in ((0, 1),):
         b1 = orc.eri_block(bs, A, B, A, B); b2 = orc.eri_block(bs, B, A, B, A).transpose(1, 0, 3, 2)
         assert float(np.abs(b1 - b2).max()) <= 2e-13 * float(np.abs(b1).max())
+
+
+@pytest.mark.parametrize("ls", [(3, 2, 3, 1), (3, 3, 3, 3), (2, 2, 2, 1)])
+def test_p9_eightfold_symmetry_d_and_f(orc, ls):
+    """P9 at d and f level on four distinct centres: the eight index permutations of (ab|cd) evaluated as eight
+    separate shell quartets (each with its own recurrence centres and HRR direction) agree to 1e-13 of the block's
+    largest element, in the fp64 core and in the long double core.  Exponents span tight and diffuse."""
+    atoms = np.array([[0.0, 0.1, -0.2], [2.9, -1.4, 0.5], [-0.6, 3.1, 1.9], [1.7, 2.8, -3.2]])
+    w = W.make_custom(atoms, [(i, ls[i]) for i in range(4)], seed=909 + sum(ls), emin=0.05, emax=500.0, nprim=4)
+    bs = orc.basis_from_workload(w)
+    for ld in (False, True):
+        ref = orc.eri_block(bs, 0, 1, 2, 3, long_double=ld).astype(np.float64)
+        scale = float(np.abs(ref).max())
+        assert scale > 1e-12
+        # (shells handed over, axes that bring the result back to [a, b, c, d] order)
+        perms = [((1, 0, 2, 3), (1, 0, 2, 3)), ((0, 1, 3, 2), (0, 1, 3, 2)), ((1, 0, 3, 2), (1, 0, 3, 2)),
+                 ((2, 3, 0, 1), (2, 3, 0, 1)), ((3, 2, 0, 1), (3, 2, 0, 1)), ((2, 3, 1, 0), (2, 3, 1, 0)),
+                 ((3, 2, 1, 0), (3, 2, 1, 0))]
+        for sh, _ in perms:
+            other = orc.eri_block(bs, *sh, long_double=ld).astype(np.float64)
+            # other[i_sh0, i_sh1, i_sh2, i_sh3]: move axis k (shell sh[k]) to position sh[k]
+            back = np.moveaxis(other, [0, 1, 2, 3], list(sh))
+            assert back.shape == ref.shape
+            assert float(np.abs(back - ref).max()) <= 1e-13 * scale, (sh, ld)
