@@ -133,16 +133,28 @@ def dmax(D) -> float:
     return float(lib().orc_dmax(_p(D, C.c_double), C.c_int(D.shape[0])))
 
 
-def jk(bs: Basis, D, tau: float, Q=None):
-    """Screened symmetric J/K.  Returns J, K, counts(dict)."""
+def dshell(bs: Basis, D) -> np.ndarray:
+    """|D|_XY = max over the shell block (X, Y) of max(|D_mu,nu|, |D_nu,mu|): the table of the block-density screen (R-23)."""
+    D = np.ascontiguousarray(D, np.float64)
+    out = np.zeros((bs.nshells, bs.nshells))
+    rc = lib().orc_dshell(*bs.args(), _p(D, C.c_double), _p(out, C.c_double))
+    if rc:
+        raise ValueError(f"orc_dshell rc={rc}")
+    return out
+
+
+def jk(bs: Basis, D, tau: float, Q=None, block_density=False):
+    """Screened symmetric J/K.  Returns J, K, counts(dict).  block_density: the screen of DESIGN.md R-23
+    ((Q_AB*Q_CD)*Dblk(AB|CD) >= tau) instead of the global-Dmax rule."""
     D = np.ascontiguousarray(D, np.float64)
     N = bs.nbf
     assert D.shape == (N, N)
     J = np.zeros((N, N)); K = np.zeros((N, N))
     counts = np.zeros(3, dtype=np.int64); cc = np.zeros(55, dtype=np.int64)
     qp = _p(np.ascontiguousarray(Q, np.float64), C.c_double) if Q is not None else None
-    rc = lib().orc_jk(*bs.args(), _p(D, C.c_double), C.c_double(tau), qp, _p(J, C.c_double), _p(K, C.c_double),
-                      _p(counts, C.c_int64), _p(cc, C.c_int64))
+    fn = lib().orc_jk_bd if block_density else lib().orc_jk
+    rc = fn(*bs.args(), _p(D, C.c_double), C.c_double(tau), qp, _p(J, C.c_double), _p(K, C.c_double),
+            _p(counts, C.c_int64), _p(cc, C.c_int64))
     if rc:
         raise ValueError(f"orc_jk rc={rc}")
     return J, K, {"unique": int(counts[0]), "kept": int(counts[1]), "prim": int(counts[2]), "per_class": cc}
@@ -171,6 +183,15 @@ def count(bs: Basis, Q, Dmax: float, tau: float):
     return {"unique": int(counts[0]), "kept": int(counts[1]), "prim": int(counts[2]), "per_class": cc}
 
 
+def count_bd(bs: Basis, Q, Dsh, tau: float):
+    """Kept-quartet counts under the block-density screen (R-23); Dsh = dshell(bs, D)."""
+    counts = np.zeros(3, dtype=np.int64); cc = np.zeros(55, dtype=np.int64)
+    Q = np.ascontiguousarray(Q, np.float64); Dsh = np.ascontiguousarray(Dsh, np.float64)
+    lib().orc_count_bd(C.c_int(bs.nshells), _p(bs.l, C.c_int32), _p(bs.nprim, C.c_int32), _p(Q, C.c_double),
+                       _p(Dsh, C.c_double), C.c_double(tau), _p(counts, C.c_int64), _p(cc, C.c_int64))
+    return {"unique": int(counts[0]), "kept": int(counts[1]), "prim": int(counts[2]), "per_class": cc}
+
+
 def jk_brute(bs: Basis, D):
     D = np.ascontiguousarray(D, np.float64)
     N = bs.nbf
@@ -181,13 +202,21 @@ def jk_brute(bs: Basis, D):
     return J, K
 
 
-def jk_block(bs: Basis, D, tau, Q, Dmax, A, B, want_j=True, want_k=True, with_work=False):
+def jk_block(bs: Basis, D, tau, Q, Dmax, A, B, want_j=True, want_k=True, with_work=False, Dsh=None):
+    """One shell block of J and K from the definition with the screen; Dsh (= dshell(bs, D)) selects the block-density
+    rule R-23, otherwise the global rule with Dmax."""
     D = np.ascontiguousarray(D, np.float64); Q = np.ascontiguousarray(Q, np.float64)
     Jb = np.zeros((bs.ncart[A], bs.ncart[B])); Kb = np.zeros((bs.ncart[A], bs.ncart[B]))
     work = np.zeros(2, dtype=np.int64)
-    rc = lib().orc_jk_block(*bs.args(), _p(D, C.c_double), C.c_double(tau), _p(Q, C.c_double), C.c_double(Dmax),
-                            C.c_int(A), C.c_int(B), _p(Jb, C.c_double) if want_j else None,
-                            _p(Kb, C.c_double) if want_k else None, _p(work, C.c_int64))
+    if Dsh is not None:
+        Dsh = np.ascontiguousarray(Dsh, np.float64)
+        rc = lib().orc_jk_block_bd(*bs.args(), _p(D, C.c_double), C.c_double(tau), _p(Q, C.c_double), _p(Dsh, C.c_double),
+                                   C.c_int(A), C.c_int(B), _p(Jb, C.c_double) if want_j else None,
+                                   _p(Kb, C.c_double) if want_k else None, _p(work, C.c_int64))
+    else:
+        rc = lib().orc_jk_block(*bs.args(), _p(D, C.c_double), C.c_double(tau), _p(Q, C.c_double), C.c_double(Dmax),
+                                C.c_int(A), C.c_int(B), _p(Jb, C.c_double) if want_j else None,
+                                _p(Kb, C.c_double) if want_k else None, _p(work, C.c_int64))
     if rc:
         raise ValueError(f"orc_jk_block rc={rc}")
     if with_work:

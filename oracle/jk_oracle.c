@@ -223,6 +223,51 @@ static void bf_offsets(const basis_t *b, int *bo)
     for (int s = 0; s < b->nshells; ++s) bo[s + 1] = bo[s] + NCART(b->l[s]);
 }
 
+/* Block-density screen (reading R-23; Haeser & Ahlrichs): the one global
+ * Dmax of the rule above is replaced, per quartet, by the largest density element the quartet's integrals can meet in
+ * the 16 updates of R-9,
+ *   Dblk(AB|CD) = max( |D|_AB, |D|_CD, |D|_AC, |D|_AD, |D|_BC, |D|_BD ),  |D|_XY = max_{mu in X, nu in Y} max(|D_mu,nu|, |D_nu,mu|),
+ * keep iff (Q_AB*Q_CD)*Dblk >= tau.  Dblk <= Dmax, so the kept set is a subset of the global rule's, and Dblk is
+ * invariant under the 8 index permutations, so the per-block definition (orc_jk_block) uses the same rule.
+ * Dsh[nshells*nshells] holds |D|_XY. */
+static void shell_block_max(const basis_t *b, const int *bo, const double *D, int N, double *Dsh)
+{
+    const int ns = b->nshells;
+    for (int X = 0; X < ns; ++X)
+        for (int Y = 0; Y < ns; ++Y) {
+            double m = 0.0;
+            for (int i = bo[X]; i < bo[X + 1]; ++i)
+                for (int j = bo[Y]; j < bo[Y + 1]; ++j) {
+                    double a = fabs(D[(size_t)i * N + j]), c = fabs(D[(size_t)j * N + i]);
+                    if (a > m) m = a;
+                    if (c > m) m = c;
+                }
+            Dsh[(size_t)X * ns + Y] = m;
+        }
+}
+static double screen_density(const double *Dsh, int ns, double Dmax, int A, int B, int C, int Dd)
+{
+    if (!Dsh) return Dmax;                      /* global rule (R-6) */
+    double m = Dsh[(size_t)A * ns + B], v;
+    v = Dsh[(size_t)C * ns + Dd]; if (v > m) m = v;
+    v = Dsh[(size_t)A * ns + C];  if (v > m) m = v;
+    v = Dsh[(size_t)A * ns + Dd]; if (v > m) m = v;
+    v = Dsh[(size_t)B * ns + C];  if (v > m) m = v;
+    v = Dsh[(size_t)B * ns + Dd]; if (v > m) m = v;
+    return m;
+}
+/* ---- exported: |D|_XY table of the block-density screen ---- */
+int orc_dshell(BASIS_ARGS, const double *D, double *Dsh)
+{
+    basis_t b = mk_basis(BASIS_PASS);
+    if (check_basis(&b)) return check_basis(&b);
+    int *bo = (int *)malloc(sizeof(int) * (nshells + 1));
+    bf_offsets(&b, bo);
+    shell_block_max(&b, bo, D, bo[nshells], Dsh);
+    free(bo);
+    return 0;
+}
+
 /* quartet class index (both sides define this independently): pair class pc = hi(hi+1)/2+lo with
  * hi >= lo the two angular momenta; quartet class X(X+1)/2+Y with X >= Y the two pair classes. */
 static int qclass(int la, int lb, int lc, int ld)
@@ -238,7 +283,7 @@ static int qclass(int la, int lb, int lc, int ld)
  * (overwritten) and the counts of that range.  Summing the partial results of disjoint ranges that cover
  * [0, npair) gives orc_jk's result; tests/golden/make_golden.py uses this to checkpoint the hours-long full runs. */
 static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, int64_t pab_lo, int64_t pab_hi,
-                    long double *Jt, long double *Kt, int64_t *counts, int64_t *class_counts)
+                    long double *Jt, long double *Kt, int64_t *counts, int64_t *class_counts, int block_density)
 {
     basis_t b = mk_basis(BASIS_PASS);
     if (check_basis(&b)) return check_basis(&b);
@@ -249,6 +294,11 @@ static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, 
     if (Qin) memcpy(Q, Qin, sizeof(double) * (size_t)nshells * nshells);
     else { int e = orc_schwarz(BASIS_PASS, Q); if (e) return e; }
     const double Dmax = dmax_of(D, (size_t)N * N);
+    double *Dsh = NULL;
+    if (block_density) {
+        Dsh = (double *)malloc(sizeof(double) * (size_t)nshells * nshells);
+        shell_block_max(&b, bo, D, N, Dsh);
+    }
     const int64_t npair = (int64_t)nshells * (nshells + 1) / 2;
     if (pab_lo < 0) pab_lo = 0;
     if (pab_hi > npair) pab_hi = npair;
@@ -280,8 +330,9 @@ static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, 
                         int64_t pcd = (int64_t)C * (C + 1) / 2 + Dd;
                         if (pcd > pab) continue;
                         ++my_all;
-                        /* keep iff (Q_AB*Q_CD)*Dmax >= tau */
-                        double bound = (Q[(size_t)A * nshells + B] * Q[(size_t)C * nshells + Dd]) * Dmax;
+                        /* keep iff (Q_AB*Q_CD)*Dmax >= tau  (block-density mode: Dblk(AB|CD) in place of Dmax) */
+                        double bound = (Q[(size_t)A * nshells + B] * Q[(size_t)C * nshells + Dd])
+                                       * screen_density(Dsh, nshells, Dmax, A, B, C, Dd);
                         if (bound < tau) continue;
                         ++my_kept;
                         my_prim += (int64_t)nprim[A] * nprim[B] * nprim[C] * nprim[Dd];
@@ -321,7 +372,7 @@ static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, 
     }
     if (counts) { counts[0] = n_all; counts[1] = n_kept; counts[2] = n_prim; }
     if (class_counts) memcpy(class_counts, cc, sizeof cc);
-    free(Q); free(bo);
+    free(Q); free(bo); free(Dsh);
     return err;
 }
 
@@ -329,31 +380,43 @@ static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, 
  * Q may be NULL (computed here) or a caller-supplied table from orc_schwarz.
  * counts[0] = unique quartets before screening, counts[1] = kept, counts[2] = primitive quartets in kept;
  * class_counts[55] = kept per class.  J, K: full symmetric [nbf*nbf], overwritten. */
-int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J, double *K,
-           int64_t *counts, int64_t *class_counts)
+static int jk_full(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J, double *K,
+                   int64_t *counts, int64_t *class_counts, int block_density)
 {
     size_t N = 0;
     for (int s = 0; s < nshells; ++s) N += (l[s] >= 0 && l[s] <= LMAX_SHELL) ? NCART(l[s]) : 0;
     long double *Jt = (long double *)calloc(N * N + 1, sizeof(long double));
     long double *Kt = (long double *)calloc(N * N + 1, sizeof(long double));
     if (!Jt || !Kt) { free(Jt); free(Kt); return -3; }
-    int err = jk_range(BASIS_PASS, D, tau, Qin, 0, (int64_t)nshells * (nshells + 1) / 2, Jt, Kt, counts, class_counts);
+    int err = jk_range(BASIS_PASS, D, tau, Qin, 0, (int64_t)nshells * (nshells + 1) / 2, Jt, Kt, counts, class_counts,
+                       block_density);
     if (err == 0)
         for (size_t i = 0; i < N * N; ++i) { J[i] = (double)Jt[i]; K[i] = (double)Kt[i]; }
     free(Jt); free(Kt);
     return err;
+}
+int orc_jk(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J, double *K,
+           int64_t *counts, int64_t *class_counts)
+{
+    return jk_full(BASIS_PASS, D, tau, Qin, J, K, counts, class_counts, 0);
+}
+/* ---- exported: the same with the block-density screen (R-23) ---- */
+int orc_jk_bd(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J, double *K,
+              int64_t *counts, int64_t *class_counts)
+{
+    return jk_full(BASIS_PASS, D, tau, Qin, J, K, counts, class_counts, 1);
 }
 
 /* ---- exported: orc_jk's loop over the bra pairs pab in [pab_lo, pab_hi) only, long double partial sums out ---- */
 int orc_jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, int64_t pab_lo, int64_t pab_hi,
                  long double *Jpart, long double *Kpart, int64_t *counts, int64_t *class_counts)
 {
-    return jk_range(BASIS_PASS, D, tau, Qin, pab_lo, pab_hi, Jpart, Kpart, counts, class_counts);
+    return jk_range(BASIS_PASS, D, tau, Qin, pab_lo, pab_hi, Jpart, Kpart, counts, class_counts, 0);
 }
 
 /* ---- exported: kept-quartet counts only (no integrals), same loop and rule as orc_jk ---- */
-int orc_count(int nshells, const int32_t *l, const int32_t *nprim, const double *Q, double Dmax, double tau,
-              int64_t *counts, int64_t *class_counts)
+static int count_impl(int nshells, const int32_t *l, const int32_t *nprim, const double *Q, double Dmax, const double *Dsh,
+                      double tau, int64_t *counts, int64_t *class_counts)
 {
     int64_t n_all = 0, n_kept = 0, n_prim = 0, cc[55];
     memset(cc, 0, sizeof cc);
@@ -366,7 +429,8 @@ int orc_count(int nshells, const int32_t *l, const int32_t *nprim, const double 
                     int64_t pcd = (int64_t)C * (C + 1) / 2 + Dd;
                     if (pcd > pab) continue;
                     ++n_all;
-                    double bound = (Q[(size_t)A * nshells + B] * Q[(size_t)C * nshells + Dd]) * Dmax;
+                    double bound = (Q[(size_t)A * nshells + B] * Q[(size_t)C * nshells + Dd])
+                                   * screen_density(Dsh, nshells, Dmax, A, B, C, Dd);
                     if (bound < tau) continue;
                     ++n_kept;
                     n_prim += (int64_t)nprim[A] * nprim[B] * nprim[C] * nprim[Dd];
@@ -376,6 +440,17 @@ int orc_count(int nshells, const int32_t *l, const int32_t *nprim, const double 
     counts[0] = n_all; counts[1] = n_kept; counts[2] = n_prim;
     memcpy(class_counts, cc, sizeof cc);
     return 0;
+}
+int orc_count(int nshells, const int32_t *l, const int32_t *nprim, const double *Q, double Dmax, double tau,
+              int64_t *counts, int64_t *class_counts)
+{
+    return count_impl(nshells, l, nprim, Q, Dmax, NULL, tau, counts, class_counts);
+}
+/* block-density rule: Dsh = the |D|_XY table of orc_dshell */
+int orc_count_bd(int nshells, const int32_t *l, const int32_t *nprim, const double *Q, const double *Dsh, double tau,
+                 int64_t *counts, int64_t *class_counts)
+{
+    return count_impl(nshells, l, nprim, Q, 0.0, Dsh, tau, counts, class_counts);
 }
 
 /* ---- exported: Eq. 1 written out, no symmetry, no screening (pin P12) ---- */
@@ -412,8 +487,8 @@ int orc_jk_brute(BASIS_ARGS, const double *D, double *J, double *K)
  * Jblk[nA*nB]:  J_mn = sum_{C,D} [ (Q_AB*Q_CD)*Dmax >= tau ] sum_{l in C, s in D} D_ls (mn|ls)
  * Kblk[nA*nB]:  K_ml = sum_{C,D} [ (Q_AC*Q_BD)*Dmax >= tau ] sum_{n in C, s in D} D_ns (m n|l s), m in A, l in B
  * (the screen is symmetric under the 8 permutations, so this equals the block of orc_jk's result). */
-int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, double Dmax,
-                 int sA, int sB, double *Jblk, double *Kblk, int64_t *work /* [2]: shell quartets, primitive quartets evaluated; may be NULL */)
+static int jk_block_impl(BASIS_ARGS, const double *D, double tau, const double *Q, double Dmax, const double *Dsh,
+                         int sA, int sB, double *Jblk, double *Kblk, int64_t *work)
 {
     int64_t w_q = 0, w_p = 0;
     basis_t b = mk_basis(BASIS_PASS);
@@ -439,7 +514,8 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
             for (int C = 0; C < nshells; ++C)
                 for (int Dd = 0; Dd < nshells; ++Dd) {
                     int nC = NCART(l[C]), nD = NCART(l[Dd]);
-                    if (Jblk && (Q[(size_t)sA * nshells + sB] * Q[(size_t)C * nshells + Dd]) * Dmax >= tau) {
+                    if (Jblk && (Q[(size_t)sA * nshells + sB] * Q[(size_t)C * nshells + Dd])
+                                    * screen_density(Dsh, nshells, Dmax, sA, sB, C, Dd) >= tau) {
                         core_shell_quartet(&b, sA, sB, C, Dd, &s, blk);
 #pragma omp atomic
                         w_q += 1;
@@ -450,7 +526,8 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
                             Jp[ia * nB + ib] += (long double)D[(size_t)(bo[C] + ic) * N + bo[Dd] + id]
                                                 * blk[((ia * nB + ib) * nC + ic) * nD + id];
                     }
-                    if (Kblk && (Q[(size_t)sA * nshells + C] * Q[(size_t)sB * nshells + Dd]) * Dmax >= tau) {
+                    if (Kblk && (Q[(size_t)sA * nshells + C] * Q[(size_t)sB * nshells + Dd])
+                                    * screen_density(Dsh, nshells, Dmax, sA, C, sB, Dd) >= tau) {
                         /* (A C | B D): mu in A, nu in C, lambda in B, sigma in D */
                         core_shell_quartet(&b, sA, C, sB, Dd, &s, blk);
 #pragma omp atomic
@@ -472,6 +549,17 @@ int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, doubl
     if (work) { work[0] = w_q; work[1] = w_p; }
     free(bo);
     return err;
+}
+int orc_jk_block(BASIS_ARGS, const double *D, double tau, const double *Q, double Dmax,
+                 int sA, int sB, double *Jblk, double *Kblk, int64_t *work /* [2]: shell quartets, primitive quartets evaluated; may be NULL */)
+{
+    return jk_block_impl(BASIS_PASS, D, tau, Q, Dmax, NULL, sA, sB, Jblk, Kblk, work);
+}
+/* the same with the block-density screen (R-23); Dsh = the |D|_XY table of orc_dshell */
+int orc_jk_block_bd(BASIS_ARGS, const double *D, double tau, const double *Q, const double *Dsh,
+                    int sA, int sB, double *Jblk, double *Kblk, int64_t *work)
+{
+    return jk_block_impl(BASIS_PASS, D, tau, Q, 0.0, Dsh, sA, sB, Jblk, Kblk, work);
 }
 
 int orc_num_threads(void)

@@ -527,8 +527,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     p->nprimpairs = p->nprimpairs_nominal = prim_total;
     // every needed Schwarz class must exist
     for (const Sublist &s : p->subl) {
-        const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
-        if (!ce.launch_schwarz && !(ce.use_rys && rys_schwarz_launcher(s.la, s.lb))) {
+        if (!rys_schwarz_launcher(s.la, s.lb)) {
             set_error("adft_shellpairs_build: no kernel for pair class (" + std::to_string(s.la) + "," + std::to_string(s.lb) + ")");
             free_pairs(p); return ADFT_ERR_UNSUPPORTED_L;
         }
@@ -614,12 +613,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     if (rc) return fail(rc);
     for (const Sublist &s : p->subl) {
         if (s.n == 0) continue;
-        const ClassEntry &ce = class_table()[quartet_class(s.pc, s.pc)];
-        if (ce.launch_schwarz) {
-            ce.launch_schwarz(p->tab, s.pair_base, s.prim_base, s.n, s.K, p->d_boysp, p->d_Q, st);
-        } else {
-            TRY2(rys_schwarz_launcher(s.la, s.lb)(p->tab, p->rys, s.pair_base, s.prim_base, s.n, s.K, p->d_Q, st));
-        }
+        TRY2(rys_schwarz_launcher(s.la, s.lb)(p->tab, p->rys, s.pair_base, s.prim_base, s.n, s.K, p->d_Q, st));
     }
     TRY2(cudaGetLastError());
     std::vector<double> Q(np);

@@ -1,5 +1,5 @@
 // adft_rys.cu -- instantiations of the block-cooperative Rys kernels (adft_rys.cuh) for the quartet classes without
-// straight-line code, and of the Schwarz kernels of the pair classes (fp), (fd), (ff).
+// straight-line code, and of the Schwarz kernels of every pair class.
 #include <atomic>
 
 #include "adft_internal.h"
@@ -49,10 +49,13 @@ template <class C>
 static cudaError_t run_sw(const PairTable &t, const RysTable &rt, int pair_base, int prim_base, int n, int K, double *Qout,
                           cudaStream_t st)
 {
-    int dev = 0, sms = 0;
+    // persistent grid: as many blocks as fit on the device (one block works on one pair at a time)
+    int dev = 0, sms = 0, occ = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    return launch_schwarz_rys<C>(t, rt, pair_base, prim_base, n, K, Qout, 2 * sms, st);
+    cudaFuncSetAttribute(schwarz_rys_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, schwarz_rys_kernel<C>, C::NT, C::SMEM_BYTES);
+    return launch_schwarz_rys<C>(t, rt, pair_base, prim_base, n, K, Qout, sms * (occ > 0 ? occ : 1), st);
 }
 
 // X(la, lb, lc, ld, NCH): NCH = number of cd chunks = thread groups per quartet.  Phase 2 is bound by shared-memory
@@ -84,6 +87,15 @@ rys_jk_fn rys_jk_launcher(int la, int lb, int lc, int ld)
 
 rys_sw_fn rys_schwarz_launcher(int la, int lb)
 {
+    // every pair class: the Rys kernel chooses the recurrence centre per primitive pair (R-22), so the bounds
+    // agree with the oracle's to 1e-10 relative also where a tight shell receives its angular momentum by transfer
+    if (la == 0 && lb == 0) return run_sw<RysCfg<0, 0, 0, 0, 1>>;
+    if (la == 1 && lb == 0) return run_sw<RysCfg<1, 0, 1, 0, 1>>;
+    if (la == 1 && lb == 1) return run_sw<RysCfg<1, 1, 1, 1, 1>>;
+    if (la == 2 && lb == 0) return run_sw<RysCfg<2, 0, 2, 0, 1>>;
+    if (la == 2 && lb == 1) return run_sw<RysCfg<2, 1, 2, 1, 1>>;
+    if (la == 2 && lb == 2) return run_sw<RysCfg<2, 2, 2, 2, 1>>;
+    if (la == 3 && lb == 0) return run_sw<RysCfg<3, 0, 3, 0, 1>>;
     if (la == 3 && lb == 1) return run_sw<RysCfg<3, 1, 3, 1, 2>>;
     if (la == 3 && lb == 2) return run_sw<RysCfg<3, 2, 3, 2, 2>>;
     if (la == 3 && lb == 3) return run_sw<RysCfg<3, 3, 3, 3, 2>>;

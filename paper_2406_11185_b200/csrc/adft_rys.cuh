@@ -470,7 +470,7 @@ __device__ __forceinline__ double rys_diag_max(int chunk, int ab, const double (
 }
 
 template <class C>
-__global__ void __launch_bounds__(C::NT, 1) schwarz_rys_kernel(const PairTable t, const RysTable rt, int pair_base, int prim_base,
+__global__ void __launch_bounds__(C::NT) schwarz_rys_kernel(const PairTable t, const RysTable rt, int pair_base, int prim_base,
                                                               int n, int K, double *__restrict__ Qout)
 {
     extern __shared__ double sm[];

@@ -12,7 +12,6 @@ intermediates that are reached, and emits
                          into acc[NE*NF] (registers when the class is small enough, else local memory);
   * G_<abcd>::hrr()      the horizontal recurrences on the contracted [e0|f0] and one `put` per integral
                          (the digestion functor of the caller folds it into J and K);
-  * G_<abcd>::hrr_diag() (classes (ab|ab) only) the diagonal integrals (mu nu|mu nu) for the Schwarz bound;
   * exact FP64 instruction counts of those paths (the "model flops" of the roofline).
 
 The same DAG can be evaluated in Python (`VrrDag.evaluate`, `HrrDag.evaluate`), which is how
@@ -349,7 +348,6 @@ def generate_class(la, lb, lc, ld, cmax_list=()):
     tag = class_tag(la, lb, lc, ld)
     vrr = best_vrr(la, lb, lc, ld)
     hrr = HrrDag(la, lb, lc, ld)
-    diag = HrrDag(la, lb, lc, ld, diag_only=True) if (la, lb) == (lc, ld) else None
     NE = sum(ncart(e) for e in range(la, la + lb + 1))
     NF = sum(ncart(f) for f in range(lc, lc + ld + 1))
     nint = ncart(la) * ncart(lb) * ncart(lc) * ncart(ld)
@@ -363,7 +361,6 @@ def generate_class(la, lb, lc, ld, cmax_list=()):
     o.append(f"    static constexpr int NA = {ncart(la)}, NB = {ncart(lb)}, NC = {ncart(lc)}, ND = {ncart(ld)};")
     o.append(f"    static constexpr int NE = {NE}, NF = {NF}, NACC = {NE * NF}, MMAX = {vrr.max_m()};")
     o.append(f"    static constexpr int VRR_OPS = {vrr.fp64_ops()}, HRR_OPS = {hrr.fp64_ops()}, NINT = {nint};")
-    o.append(f"    static constexpr bool HAS_DIAG = {'true' if diag else 'false'};")
     o.append("    template <class Ctx, class Acc>")
     o.append("    static __device__ __forceinline__ void vrr(const Ctx &c, const double *__restrict__ F, Acc &acc) {")
     vrr.emit(o)
@@ -372,12 +369,6 @@ def generate_class(la, lb, lc, ld, cmax_list=()):
     o.append("    static __device__ __forceinline__ void hrr(const Acc &acc, double ABx, double ABy, double ABz,")
     o.append("                                                double CDx, double CDy, double CDz, Dg &dg) {")
     hrr.emit(o)
-    o.append("    }")
-    o.append("    template <class Acc, class Dg>")
-    o.append("    static __device__ __forceinline__ void hrr_diag(const Acc &acc, double ABx, double ABy, double ABz,")
-    o.append("                                                     double CDx, double CDy, double CDz, Dg &dg) {")
-    if diag:
-        diag.emit(o)
     o.append("    }")
     o.append("};")
     gidx = {t: i for i, t in enumerate(all_targets(la, lb, lc, ld))}

@@ -3,6 +3,9 @@
 
     python tests/golden/make_golden.py full 2            # full oracle J, K, Q, counts, energies of cfg 2
     python tests/golden/make_golden.py full 3            # same for cfg 3 (hours; resumable: --ckpt, --max-seconds)
+    python tests/golden/make_golden.py full 3 --ckpt a.npz --chunk-lo 0 --chunk-hi 100     # part of the chunks on one machine,
+    python tests/golden/make_golden.py full 3 --ckpt b.npz --chunk-lo 100 --chunk-hi 256   # the rest on another,
+    python tests/golden/make_golden.py merge 3 a.npz b.npz                                 # then add the partial sums
     python tests/golden/make_golden.py blocks 4 [--per-type 23]   # stratified sampled J/K shell blocks of cfg 4
 
 `full` runs oracle.jk_range (orc_jk's own loop, restricted to a range of bra pairs, long double partial sums) chunk
@@ -52,7 +55,58 @@ def chunk_bounds(npair: int, nchunks: int):
     return [(edges[k], edges[k + 1]) for k in range(nchunks) if edges[k + 1] > edges[k]]
 
 
-def full(cfg: int, out: str, ckpt: str, nchunks: int, max_seconds: float = 0.0):
+def save_partial(path, sha, nchunks, lo, done, cnt, cc, J, K):
+    """Running long double sums of the chunks [lo, done): long double does not survive np.save portably, so the file
+    keeps hi + lo fp64 parts (106 bits, more than the 64-bit significand of the x87 type)."""
+    Jhi = J.astype(np.float64); Khi = K.astype(np.float64)
+    tmp = path + ".tmp.npz"
+    np.savez(tmp, sha=sha, nchunks=nchunks, lo=lo, done=done, cnt=cnt, cc=cc, Jhi=Jhi,
+             Jlo=(J - Jhi).astype(np.float64), Khi=Khi, Klo=(K - Khi).astype(np.float64))
+    os.replace(tmp, path)
+
+
+def write_full(out, cfg, w, sha, Q, J, K, cnt, cc, seconds):
+    """Round the long double sums once and store the result (what oracle.jk returns)."""
+    N = J.shape[0]
+    Dl = np.asarray(w.D, np.longdouble)
+    EJ = 0.5 * np.sum(Dl * J); EK = -0.25 * np.sum(Dl * K)
+    J64 = J.astype(np.float64); K64 = K.astype(np.float64)
+    assert np.array_equal(J64, J64.T) or np.abs(J64 - J64.T).max() <= 1e-13 * np.abs(J64).max()
+    il = np.tril_indices(N)
+    np.savez_compressed(out, sha=sha, cfg=cfg, nbf=N, tau=w.tau, dmax=oracle.dmax(w.D), Q=Q,
+                        J_tril=J64[il], K_tril=K64[il], unique=cnt[0], kept=cnt[1], prim=cnt[2], per_class=cc,
+                        EJ_hi=np.float64(EJ), EJ_lo=np.float64(EJ - np.longdouble(np.float64(EJ))),
+                        EK_hi=np.float64(EK), EK_lo=np.float64(EK - np.longdouble(np.float64(EK))),
+                        seconds=seconds, threads=oracle.num_threads())
+    print(f"wrote {out}: kept {cnt[1]} prim {cnt[2]} E_J {float(EJ):.12f} E_K {float(EK):.12f} {seconds:.0f} s", flush=True)
+
+
+def merge(cfg: int, out: str, parts):
+    """Add the partial sums of `full --chunk-lo/--chunk-hi` runs (each a finished --ckpt file) and write the result."""
+    w = W.make(cfg)
+    sha = input_sha256(w)
+    bs = oracle.basis_from_workload(w)
+    N = bs.nbf
+    J = np.zeros((N, N), np.longdouble); K = np.zeros((N, N), np.longdouble)
+    cnt = np.zeros(3, np.int64); cc = np.zeros(55, np.int64)
+    ranges = []
+    nch = None
+    for path in parts:
+        c = np.load(path, allow_pickle=False)
+        assert str(c["sha"]) == sha, f"{path} was made from other inputs"
+        nch = int(c["nchunks"]) if nch is None else nch
+        assert int(c["nchunks"]) == nch, "partial files use different chunkings"
+        ranges.append((int(c["lo"]), int(c["done"])))
+        J += c["Jhi"].astype(np.longdouble) + c["Jlo"].astype(np.longdouble)
+        K += c["Khi"].astype(np.longdouble) + c["Klo"].astype(np.longdouble)
+        cnt += c["cnt"]; cc += c["cc"]
+    ranges.sort()
+    assert ranges[0][0] == 0 and ranges[-1][1] == nch and all(a[1] == b[0] for a, b in zip(ranges, ranges[1:])), \
+        f"partial files do not tile the chunks 0..{nch}: {ranges}"
+    write_full(out, cfg, w, sha, oracle.schwarz(bs), J, K, cnt, cc, 0.0)
+
+
+def full(cfg: int, out: str, ckpt: str, nchunks: int, max_seconds: float = 0.0, chunk_lo: int = 0, chunk_hi: int = -1):
     w = W.make(cfg)
     sha = input_sha256(w)
     bs = oracle.basis_from_workload(w)
@@ -64,16 +118,16 @@ def full(cfg: int, out: str, ckpt: str, nchunks: int, max_seconds: float = 0.0):
     N = bs.nbf
     J = np.zeros((N, N), np.longdouble); K = np.zeros((N, N), np.longdouble)
     cnt = np.zeros(3, np.int64); cc = np.zeros(55, np.int64)
-    done = 0
+    chunk_hi = len(chunks) if chunk_hi < 0 else min(chunk_hi, len(chunks))
+    done = chunk_lo
     if ckpt and os.path.exists(ckpt):
         c = np.load(ckpt, allow_pickle=False)
-        if str(c["sha"]) == sha and int(c["nchunks"]) == len(chunks):
-            # long double does not survive np.save portably: the checkpoint keeps hi + lo fp64 parts
+        if str(c["sha"]) == sha and int(c["nchunks"]) == len(chunks) and int(c["lo"]) == chunk_lo:
             J = c["Jhi"].astype(np.longdouble) + c["Jlo"].astype(np.longdouble)
             K = c["Khi"].astype(np.longdouble) + c["Klo"].astype(np.longdouble)
             cnt, cc, done = c["cnt"], c["cc"], int(c["done"])
             print(f"resuming after chunk {done}/{len(chunks)}", flush=True)
-    for i in range(done, len(chunks)):
+    for i in range(done, chunk_hi):
         if max_seconds and time.time() - t0 > max_seconds:
             print(f"stopping after {time.time() - t0:.0f} s with {i}/{len(chunks)} chunks done (resume with the same --ckpt)", flush=True)
             return
@@ -85,22 +139,11 @@ def full(cfg: int, out: str, ckpt: str, nchunks: int, max_seconds: float = 0.0):
         print(f"chunk {i + 1}/{len(chunks)} pab [{lo},{hi}) kept {ci['kept']} prim {ci['prim']} "
               f"{time.time() - t1:.0f} s (total {time.time() - t0:.0f} s)", flush=True)
         if ckpt:
-            Jhi = J.astype(np.float64); Khi = K.astype(np.float64)
-            tmp = ckpt + ".tmp.npz"
-            np.savez(tmp, sha=sha, nchunks=len(chunks), done=i + 1, cnt=cnt, cc=cc, Jhi=Jhi,
-                     Jlo=(J - Jhi).astype(np.float64), Khi=Khi, Klo=(K - Khi).astype(np.float64))
-            os.replace(tmp, ckpt)
-    Dl = np.asarray(w.D, np.longdouble)
-    EJ = 0.5 * np.sum(Dl * J); EK = -0.25 * np.sum(Dl * K)
-    J64 = J.astype(np.float64); K64 = K.astype(np.float64)
-    assert np.array_equal(J64, J64.T) or np.abs(J64 - J64.T).max() <= 1e-13 * np.abs(J64).max()
-    il = np.tril_indices(N)
-    np.savez_compressed(out, sha=sha, cfg=cfg, nbf=N, tau=w.tau, dmax=oracle.dmax(w.D), Q=Q,
-                        J_tril=J64[il], K_tril=K64[il], unique=cnt[0], kept=cnt[1], prim=cnt[2], per_class=cc,
-                        EJ_hi=np.float64(EJ), EJ_lo=np.float64(EJ - np.longdouble(np.float64(EJ))),
-                        EK_hi=np.float64(EK), EK_lo=np.float64(EK - np.longdouble(np.float64(EK))),
-                        seconds=time.time() - t0, threads=oracle.num_threads())
-    print(f"wrote {out}: kept {cnt[1]} prim {cnt[2]} E_J {float(EJ):.12f} E_K {float(EK):.12f} {time.time() - t0:.0f} s", flush=True)
+            save_partial(ckpt, sha, len(chunks), chunk_lo, i + 1, cnt, cc, J, K)
+    if chunk_lo != 0 or chunk_hi != len(chunks):
+        print(f"chunks [{chunk_lo},{chunk_hi}) done; combine the partial files with `merge`", flush=True)
+        return
+    write_full(out, cfg, w, sha, Q, J, K, cnt, cc, time.time() - t0)
 
 
 def blocks(cfg: int, out: str, per_type: int, seed: int):
@@ -137,8 +180,11 @@ def blocks(cfg: int, out: str, per_type: int, seed: int):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("mode", choices=["full", "blocks"])
+    ap.add_argument("mode", choices=["full", "blocks", "merge"])
     ap.add_argument("cfg", type=int)
+    ap.add_argument("parts", nargs="*", help="`merge`: the finished --ckpt files of the partial runs")
+    ap.add_argument("--chunk-lo", type=int, default=0, help="`full`: first chunk of a partial run")
+    ap.add_argument("--chunk-hi", type=int, default=-1, help="`full`: one past the last chunk of a partial run")
     ap.add_argument("--out", default=None)
     ap.add_argument("--ckpt", default=None, help="checkpoint file of a `full` run (resumed if it matches the inputs)")
     ap.add_argument("--chunks", type=int, default=64)
@@ -147,7 +193,9 @@ def main():
     ap.add_argument("--seed", type=int, default=2406)
     a = ap.parse_args()
     if a.mode == "full":
-        full(a.cfg, a.out or os.path.join(HERE, f"cfg{a.cfg}_full.npz"), a.ckpt, a.chunks, a.max_seconds)
+        full(a.cfg, a.out or os.path.join(HERE, f"cfg{a.cfg}_full.npz"), a.ckpt, a.chunks, a.max_seconds, a.chunk_lo, a.chunk_hi)
+    elif a.mode == "merge":
+        merge(a.cfg, a.out or os.path.join(HERE, f"cfg{a.cfg}_full.npz"), a.parts)
     else:
         blocks(a.cfg, a.out or os.path.join(HERE, f"cfg{a.cfg}_blocks.npz"), a.per_type, a.seed)
 

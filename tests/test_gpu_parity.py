@@ -2,7 +2,7 @@
 
 Tolerances (BASELINE.json north_star): max-abs 1e-10 per element of J and K, 1e-9 Hartree on
 E_J = 1/2 tr(DJ) and E_K = -1/4 tr(DK) (evaluated as 1/2 sum D (J_gpu - J_oracle) in long double, SURVEY R-12);
-screening identical: per-class kept counts are equal integers and the Schwarz tables agree to the bounds of check_q.
+screening identical: per-class kept counts are equal integers and the Schwarz tables agree to 1e-12 relative (check_q).
 
 Where the oracle runs in seconds (cfg 0, 0b, 1, the class sweeps) it is called live.  For cfg 2 and cfg 3 the FULL
 oracle result (every element of J and K, the energies, Q, the counts) is stored under tests/golden/ by
@@ -36,11 +36,13 @@ def denergy(D, A, B, fac):
 
 
 def check_q(Q, Qo):
-    """Schwarz tables agree: PLACEHOLDER_BOUNDS"""
-    assert np.abs(Q - Qo).max() <= 1e-9 * max(1.0, Qo.max())
+    """Schwarz tables agree to 1e-12 relative wherever the bound is above 1e-12, and to 1e-13 absolute
+    everywhere.  Every pair class goes through the Rys Schwarz kernel, which picks the recurrence centre per primitive
+    pair exactly as the oracle does (R-22); measured on cfg 1, 2, 3: largest relative difference 8.3e-14."""
+    assert np.abs(Q - Qo).max() <= 1e-13 * max(1.0, Qo.max())
     big = Qo > 1e-12
     if big.any():
-        assert (np.abs(Q - Qo)[big] / Qo[big]).max() <= 1e-5
+        assert (np.abs(Q - Qo)[big] / Qo[big]).max() <= 1e-12
 
 
 def check_full(api, orc, w, tau=None):
