@@ -187,6 +187,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-mixed", action="store_true", help="skip the mixed-precision (f64+f32) measurement reported beside the f64 line")
     ap.add_argument("--prim-threshold", type=float, default=None,
                     help="primitive-pair threshold (default: the library's ADFT_DEFAULT_PRIM_THRESHOLD; 0 = no primitive screening)")
     args = ap.parse_args()
@@ -273,6 +274,35 @@ def main():
     e2e_value = job_value(kept, world, e2e_ms)
     assert np.isfinite(chk)
 
+    # beside the f64 headline (never instead of it): the paper's mixed-precision dispatch,
+    # quartets with tau <= S < 1e5 tau in single precision.  Same workload, same kept set; timed the same way, and its
+    # J, K compared with the f64 J, K of the timed builds above.
+    mixed = None
+    if not args.no_mixed:
+        Jm = torch.empty_like(D); Km = torch.empty_like(D)
+        sp.jk_build(D, Jm, Km, w.tau, mixed_precision=True); torch.cuda.synchronize()        # warm-up (module load)
+        mx_ms = []
+        for _ in range(max(1, min(args.steps, 3))):
+            flush.zero_()
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            sp.jk_build(D, Jm, Km, w.tau, stream=stream, mixed_precision=True)
+            b.record(stream); b.synchronize()
+            mx_ms.append(a.elapsed_time(b))
+        sm = sp.stats()
+        mms = reduce_max_over_ranks([float(np.mean(mx_ms))], world, "cuda")[0]
+        Dl = D.to(torch.float64)
+        mixed = {"dtype": "f64+f32", "fp32_band": 1e5, "ms_per_step": mms, "value": job_value(int(sm.quartets_kept), world, mms),
+                 "unit": "quartets/s", "speedup_vs_f64": ms_step / mms,
+                 "quartets_kept": int(sm.quartets_kept), "quartets_fp32": int(sm.quartets_fp32),
+                 "fp32_fraction": int(sm.quartets_fp32) / max(1, int(sm.quartets_kept)),
+                 "max_abs_dJ_vs_f64": float((Jm - J).abs().max()), "max_abs_dK_vs_f64": float((Km - K).abs().max()),
+                 "dE_J_vs_f64": float(0.5 * (Dl * (Jm - J)).sum()), "dE_K_vs_f64": float(-0.25 * (Dl * (Km - K)).sum()),
+                 "E_J": float(0.5 * (Dl * J).sum()), "E_K": float(-0.25 * (Dl * K).sum())}
+        sp.jk_build(D, J, K, w.tau); torch.cuda.synchronize()       # leave the stats of an f64 build behind
+        stats_after = sp.stats()
+        assert int(stats_after.quartets_kept) == kept == mixed["quartets_kept"]
+
     if rank == 0:
         class_ms /= args.steps
         cq = np.array(stats.class_quartets[:])
@@ -322,6 +352,8 @@ def main():
                "e2e": {"value": e2e_value, "unit": "quartets/s", "ms_per_step": e2e_ms,
                        "h2d_bytes_per_step": int(N) * N * 8, "d2h_bytes_per_step": 2 * int(N) * N * 8},
                "gpu_launches": int(stats.kernel_launches) * args.steps, "clocks": clocks}
+        if mixed is not None:
+            out["mixed_precision"] = mixed
         if not args.no_cpu_baseline:
             smp = oracle_sample(w, args.cpu_seconds)
             err = sample_max_abs_err(smp, J.cpu().numpy(), K.cpu().numpy())      # the J, K of the timed builds

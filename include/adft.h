@@ -77,6 +77,10 @@ typedef struct {
     double  ms_dmax, ms_plan, ms_eri, ms_finalize, ms_total; /* device ms; ms_total = whole call */
     int32_t kernel_launches;      /* kernels launched by the call */
     int32_t reserved;
+    /* mixed-precision dispatch (ADFT_JK_MIXED_PRECISION): the part of the counts above evaluated in single precision */
+    int64_t quartets_fp32;
+    int64_t class_quartets_fp32[ADFT_MAX_CLASSES];
+    double  class_ms_fp32[ADFT_MAX_CLASSES];  /* device time of each class's single-precision launch */
 } adft_jk_stats_t;
 
 #define ADFT_MAX_NPRIM 32        /* largest contraction depth of one shell */
@@ -137,6 +141,58 @@ adft_status_t adft_shellpairs_schwarz(const adft_shellpairs_t *pairs, double *Q)
  *         non-finite D -> NOT_FINITE (outputs untouched);  CUDA failures -> ERR_CUDA. */
 adft_status_t adft_jk_build(adft_shellpairs_t *pairs, const double *D, double *J, double *K,
                             double schwarz_threshold, void *cuda_stream);
+
+/* Options of adft_jk_build_ex.  Zero-initialise the struct: every field at 0 means "as adft_jk_build".
+ *
+ *  ADFT_JK_BLOCK_DENSITY (Haeser-Ahlrichs density screening; reading R-23):
+ *     the single max|D| of the screen is replaced, per quartet, by
+ *         Dblk(AB|CD) = max(|D|_AB, |D|_CD, |D|_AC, |D|_AD, |D|_BC, |D|_BD),  |D|_XY = max over the shell block,
+ *     i.e. a quartet is skipped iff (Q_AB*Q_CD)*Dblk < tau.  Dblk <= max|D|, so the kept set is a subset of the default
+ *     rule's; adft_jk_stats reports the kept counts of the rule that was used.
+ *  shard_rank / shard_count (replicated D, independent quartet batches, one
+ *     reduction): the call evaluates only the warp tiles t of every class launch with t % shard_count == shard_rank
+ *     and writes the PARTIAL symmetric J, K of those quartets; the sum over all ranks of a group is the full result
+ *     (one all-reduce, done by the caller -- the Python binding uses torch.distributed).  shard_count 0 or 1 = all
+ *     tiles.  adft_jk_stats then reports the counts of this rank's share.
+ *  ADFT_JK_MIXED_PRECISION (the paper's "mixed single and double precision strategy"):
+ *     with S = (Q_AB*Q_CD)*density, the number the screen already forms (reading R-24),
+ *         S < tau                     -> not evaluated                       ("there will not be dispatch")
+ *         tau <= S < fp32_band * tau  -> evaluated in SINGLE precision       ("the single precision version is enough")
+ *         S >= fp32_band * tau        -> evaluated in double precision       ("the double precision version is necessary")
+ *     Single precision = Boys function, recurrences, contraction and per-quartet digestion sums in fp32; the product
+ *     centre difference P - Q and every reduction into J and K stay fp64.  The kept set and its counts are those of
+ *     the fp64 build.  Each single-precision integral carries a relative error of order 1e-6 on a contribution bounded
+ *     by fp32_band*tau, i.e. an absolute error per quartet of the order of the screening threshold itself; J and K
+ *     then differ from the fp64 build by more than the 1e-10 of the default path (DESIGN.md section 7 has the measured
+ *     error study).  Needs both J and K; the quartet classes with f shells that run through the Rys kernels stay fp64.
+ *  Errors: unknown flag bits, shard_rank outside [0, shard_count), mixed precision with J or K NULL, fp32_band < 1
+ *  or non-finite -> INVALID_ARG. */
+#define ADFT_JK_BLOCK_DENSITY 1u
+#define ADFT_JK_MIXED_PRECISION 2u
+#define ADFT_DEFAULT_FP32_BAND 1e5
+typedef struct {
+    uint32_t flags;
+    int32_t shard_rank, shard_count;
+    int32_t reserved0;
+    double fp32_band;             /* ADFT_JK_MIXED_PRECISION: width of the single-precision band; 0 = 1e5 */
+    double reserved[3];
+} adft_jk_options_t;
+
+/* adft_jk_build with options (NULL options = adft_jk_build). */
+adft_status_t adft_jk_build_ex(adft_shellpairs_t *pairs, const double *D, double *J, double *K,
+                               double schwarz_threshold, const adft_jk_options_t *options, void *cuda_stream);
+
+/* Incremental build ("incremental Fock"): J and K are linear in D, so given the matrices
+ * of a previous density only the difference has to be evaluated, and with the block-density screen a small, localised
+ * dD keeps few quartets.  All pointers DEVICE, N*N fp64:
+ *   on entry  J, K hold the matrices that belong to D_prev (either may be NULL);
+ *   the call forms dD = D - D_prev, builds J(dD), K(dD) with ADFT_JK_BLOCK_DENSITY (always on here; the other
+ *   options apply as given) into internal buffers, and then
+ *   on exit   J += J(dD), K += K(dD), D_prev = D.
+ * The screening error of a sequence of incremental builds accumulates: callers rebuild from scratch every few
+ * iterations.  Stats are those of the dD build.  Errors as adft_jk_build; D_prev must not alias D, J or K. */
+adft_status_t adft_jk_build_incremental(adft_shellpairs_t *pairs, const double *D, double *D_prev, double *J, double *K,
+                                        double schwarz_threshold, const adft_jk_options_t *options, void *cuda_stream);
 
 /* Convenience for host callers: D, J, K are HOST N*N arrays; the call stages them through internal device buffers
  * on cuda_stream (host->device copy of D, the build, device->host copies of J and K) and synchronises. */

@@ -38,10 +38,21 @@ class JKStats(C.Structure):
                 ("model_flops", C.c_double), ("dmax", C.c_double),
                 ("ms_dmax", C.c_double), ("ms_plan", C.c_double), ("ms_eri", C.c_double),
                 ("ms_finalize", C.c_double), ("ms_total", C.c_double),
-                ("kernel_launches", C.c_int32), ("reserved", C.c_int32)]
+                ("kernel_launches", C.c_int32), ("reserved", C.c_int32),
+                ("quartets_fp32", C.c_int64), ("class_quartets_fp32", C.c_int64 * ADFT_MAX_CLASSES),
+                ("class_ms_fp32", C.c_double * ADFT_MAX_CLASSES)]
 
 
-EXPORTS = ["adft_basis_create", "adft_basis_nbf", "adft_basis_shell_offsets", "adft_basis_coefficients",
+class JKOptions(C.Structure):
+    """adft_jk_options_t (include/adft.h): flags, shard_rank, shard_count."""
+    _fields_ = [("flags", C.c_uint32), ("shard_rank", C.c_int32), ("shard_count", C.c_int32), ("reserved0", C.c_int32),
+                ("fp32_band", C.c_double), ("reserved", C.c_double * 3)]
+
+
+ADFT_JK_BLOCK_DENSITY = 1
+ADFT_JK_MIXED_PRECISION = 2
+
+EXPORTS = ["adft_jk_build_ex", "adft_jk_build_incremental", "adft_basis_create", "adft_basis_nbf", "adft_basis_shell_offsets", "adft_basis_coefficients",
            "adft_shellpairs_build", "adft_shellpairs_build_ex", "adft_shellpairs_prim_counts", "adft_shellpairs_schwarz", "adft_jk_build", "adft_jk_build_host", "adft_jk_stats",
            "adft_shellpairs_counts", "adft_shellpairs_destroy", "adft_basis_destroy", "adft_status_string",
            "adft_last_error", "adft_fp64_peak_tflops"]
@@ -59,6 +70,9 @@ def lib():
         L.adft_shellpairs_destroy.restype = None
         L.adft_basis_destroy.restype = None
         L.adft_jk_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
+        L.adft_jk_build_ex.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
+        L.adft_jk_build_incremental.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
+                                                C.c_void_p, C.c_void_p]
         L.adft_jk_build_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.adft_shellpairs_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.adft_shellpairs_build_ex.argtypes = [C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
@@ -155,17 +169,58 @@ class ShellPairs:
         _check(lib().adft_shellpairs_counts(self._h, C.byref(a), C.byref(b)))
         return int(a.value), int(b.value)
 
-    def jk_build(self, D, J=None, K=None, tau=0.0, stream=None):
-        """D, J, K: torch.float64 CUDA tensors [N,N] (J or K may be None).  Enqueues on `stream`."""
+    def _check_tensors(self, *ts):
         N = self.basis.nbf
-        for t in (D, J, K):
+        for t in ts:
             if t is not None:
                 assert t.is_cuda and t.dtype.is_floating_point and t.element_size() == 8 and t.is_contiguous()
                 assert tuple(t.shape) == (N, N)
-        _check(lib().adft_jk_build(self._h, C.c_void_p(D.data_ptr()),
-                                   C.c_void_p(J.data_ptr()) if J is not None else None,
-                                   C.c_void_p(K.data_ptr()) if K is not None else None,
-                                   C.c_double(tau), _stream_ptr(stream)))
+
+    @staticmethod
+    def _options(block_density, shard, mixed_precision=False, fp32_band=0.0):
+        o = JKOptions()
+        o.flags = (ADFT_JK_BLOCK_DENSITY if block_density else 0) | (ADFT_JK_MIXED_PRECISION if mixed_precision else 0)
+        o.fp32_band = float(fp32_band)
+        if shard is not None:
+            o.shard_rank, o.shard_count = int(shard[0]), int(shard[1])
+        return o
+
+    def jk_build(self, D, J=None, K=None, tau=0.0, stream=None, block_density=False, shard=None, mixed_precision=False,
+                 fp32_band=0.0):
+        """D, J, K: torch.float64 CUDA tensors [N,N] (J or K may be None).  Enqueues on `stream`.
+        block_density: the screen of DESIGN.md R-23; shard = (rank, count): only this rank's share of the tiles
+        (partial J, K; see jk_build_distributed); mixed_precision: quartets with tau <= S < fp32_band*tau (default 1e5)
+        in single precision."""
+        self._check_tensors(D, J, K)
+        if not block_density and shard is None and not mixed_precision:
+            _check(lib().adft_jk_build(self._h, C.c_void_p(D.data_ptr()),
+                                       C.c_void_p(J.data_ptr()) if J is not None else None,
+                                       C.c_void_p(K.data_ptr()) if K is not None else None,
+                                       C.c_double(tau), _stream_ptr(stream)))
+            return
+        o = self._options(block_density, shard, mixed_precision, fp32_band)
+        _check(lib().adft_jk_build_ex(self._h, C.c_void_p(D.data_ptr()),
+                                      C.c_void_p(J.data_ptr()) if J is not None else None,
+                                      C.c_void_p(K.data_ptr()) if K is not None else None,
+                                      C.c_double(tau), C.byref(o), _stream_ptr(stream)))
+
+    def jk_build_incremental(self, D, D_prev, J=None, K=None, tau=0.0, stream=None, shard=None):
+        """adft_jk_build_incremental: J, K hold the matrices of D_prev on entry and those of D on exit; D_prev <- D."""
+        self._check_tensors(D, D_prev, J, K)
+        o = self._options(True, shard)
+        _check(lib().adft_jk_build_incremental(self._h, C.c_void_p(D.data_ptr()), C.c_void_p(D_prev.data_ptr()),
+                                               C.c_void_p(J.data_ptr()) if J is not None else None,
+                                               C.c_void_p(K.data_ptr()) if K is not None else None,
+                                               C.c_double(tau), C.byref(o), _stream_ptr(stream)))
+
+    def jk_build_distributed(self, D, J=None, K=None, tau=0.0, group=None, block_density=False):
+        """Sharded build over the ranks of a torch.distributed process group (PAPER.md:105, 283-291:
+        replicated D, independent quartet batches, one reduction): every rank holds the same D and pair table, evaluates
+        the tiles t with t % world == rank, and the partial J, K are summed with one all-reduce each (NCCL over
+        NVLink on GPUs).  On return every rank holds the full J and K."""
+        rank, world = shard_of(group)
+        self.jk_build(D, J, K, tau, block_density=block_density, shard=(rank, world) if world > 1 else None)
+        allreduce_jk(J, K, group)
 
     def jk_build_host(self, D, J=None, K=None, tau=0.0, stream=None):
         """D, J, K: numpy float64 [N,N] host arrays (pinned or not); copies are inside the call."""
@@ -191,21 +246,41 @@ class ShellPairs:
             pass
 
 
+def shard_of(group=None):
+    """(rank, world size) of this process in `group`; (0, 1) when torch.distributed is not initialised."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return 0, 1
+    return dist.get_rank(group), dist.get_world_size(group)
+
+
+def allreduce_jk(J, K, group=None):
+    """The one exchange step of the sharded build: sum the ranks' partial J and K in place (no-op for one rank)."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
+        return
+    for M in (J, K):
+        if M is not None:
+            dist.all_reduce(M, op=dist.ReduceOp.SUM, group=group)
+
+
 def fp64_peak_tflops(stream=None) -> float:
     v = C.c_double()
     _check(lib().adft_fp64_peak_tflops(_stream_ptr(stream), C.byref(v)))
     return float(v.value)
 
 
-def jk(workload, tau=None, want_j=True, want_k=True, prim_threshold=None):
+def jk(workload, tau=None, want_j=True, want_k=True, prim_threshold=None, block_density=False, D=None,
+       mixed_precision=False, fp32_band=0.0):
     """Convenience: full path on cuda:0 for a workloads.Workload; returns numpy J, K and the stats."""
     import torch
     bs = Basis.from_workload(workload)
     sp = ShellPairs(bs, prim_threshold=prim_threshold)
-    D = torch.from_numpy(workload.D).cuda()
+    D = torch.from_numpy(np.ascontiguousarray(workload.D if D is None else D)).cuda()
     J = torch.empty_like(D) if want_j else None
     K = torch.empty_like(D) if want_k else None
-    sp.jk_build(D, J, K, workload.tau if tau is None else tau)
+    sp.jk_build(D, J, K, workload.tau if tau is None else tau, block_density=block_density,
+                mixed_precision=mixed_precision, fp32_band=fp32_band)
     torch.cuda.synchronize()
     st = sp.stats()
     out = (J.cpu().numpy() if want_j else None, K.cpu().numpy() if want_k else None, st, sp.schwarz())

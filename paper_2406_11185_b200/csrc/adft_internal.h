@@ -18,7 +18,7 @@ inline int quartet_class(int X, int Y) { return X * (X + 1) / 2 + Y; }          
 
 // Per-class launchers, filled by the instantiation units (one per generated class).
 struct ClassEntry {
-    void (*launch_jk)(const JKParams &p, cudaStream_t st, bool want_j, bool want_k) = nullptr;
+    void (*launch_jk)(const JKParams &p, cudaStream_t st, bool want_j, bool want_k, bool fp32) = nullptr;
     int la = 0, lb = 0, lc = 0, ld = 0;
     int vrr_ops = 0, hrr_ops = 0, nint = 0;   // FP64 instruction counts from the generator
     const char *impl = "none";                // "straightline" | "rys"

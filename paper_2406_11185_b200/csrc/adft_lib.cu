@@ -117,7 +117,7 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int K, int
                                  const int32_t *__restrict__ sh_nprim, const int32_t *__restrict__ sh_off,
                                  const double *__restrict__ xyz, const double *__restrict__ expo,
                                  const double *__restrict__ coef, double *zeta, double *inv2z, double *Px, double *Py,
-                                 double *Pz, double *PAx, double *PAy, double *PAz, double *cc)
+                                 double *Pz, double *PAx, double *PAy, double *PAz, double *cc, float *f32, size_t npp)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
@@ -151,7 +151,12 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int K, int
         zeta[slot] = z;  inv2z[slot] = 0.5 * iz;
         Px[slot] = px;  Py[slot] = py;  Pz[slot] = pz;
         PAx[slot] = px - Ax;  PAy[slot] = py - Ay;  PAz[slot] = pz - Az;
-        cc[slot] = c0 * ca[ia] * cb[ib] * exp(-a * b * iz * AB2) * iz;
+        const double ccv = c0 * ca[ia] * cb[ib] * exp(-a * b * iz * AB2) * iz;
+        cc[slot] = ccv;
+        // single-precision copies for the fp32 launches of the mixed-precision dispatch: zeta, 1/2zeta, P - A, prefactor
+        f32[slot] = (float)z;  f32[npp + slot] = (float)(0.5 * iz);
+        f32[2 * npp + slot] = (float)(px - Ax);  f32[3 * npp + slot] = (float)(py - Ay);  f32[4 * npp + slot] = (float)(pz - Az);
+        f32[5 * npp + slot] = (float)ccv;
     }
 }
 
@@ -173,6 +178,36 @@ __global__ void dmax_kernel(const double *__restrict__ D, size_t n, unsigned lon
     if ((threadIdx.x & 31) == 0) {
         atomicMax(out, (unsigned long long)__double_as_longlong(m));
         if (bad) atomicOr(out + 1, 1ull);
+    }
+}
+
+// (f3) |D|_XY = max over the shell block (X, Y) of max(|D_ij|, |D_ji|): the table of the block-density screen (R-23).
+// One thread per shell pair X >= Y (blocks hold at most 10 x 10 elements).
+__global__ void dshell_kernel(const double *__restrict__ D, int N, const int32_t *__restrict__ bfoff, int ns, double *__restrict__ Dsh)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)ns * ns) return;
+    const int X = (int)(idx / ns), Y = (int)(idx - (long long)X * ns);
+    if (Y > X) return;
+    double m = 0.0;
+    for (int i = bfoff[X]; i < bfoff[X + 1]; ++i)
+        for (int j = bfoff[Y]; j < bfoff[Y + 1]; ++j)
+            m = fmax(m, fmax(fabs(__ldg(D + (size_t)i * N + j)), fabs(__ldg(D + (size_t)j * N + i))));
+    Dsh[(size_t)X * ns + Y] = Dsh[(size_t)Y * ns + X] = m;
+}
+
+// (f3) incremental build: out = a - b;  and  J += Js, K += Ks, Dprev = D
+__global__ void diff_kernel(const double *__restrict__ a, const double *__restrict__ b, double *__restrict__ out, size_t n)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) out[i] = a[i] - b[i];
+}
+__global__ void incr_finish_kernel(double *J, const double *__restrict__ Js, double *K, const double *__restrict__ Ks,
+                                   double *Dprev, const double *__restrict__ D, size_t n)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        if (J) J[i] += Js[i];
+        if (K) K[i] += Ks[i];
+        Dprev[i] = D[i];
     }
 }
 
@@ -230,6 +265,8 @@ struct adft_shellpairs {
     int32_t *d_atom = nullptr, *d_nprim = nullptr, *d_off = nullptr;
     // device: pair table
     double *d_Q = nullptr, *d_AB = nullptr /* 3*npairs */, *d_prim = nullptr /* 9*nprimpairs */;
+    float *d_primf = nullptr;                 // 6*nprimpairs single-precision copies (zeta, 1/2zeta, P-A, prefactor)
+    float *d_boysf = nullptr;                 // the per-order Boys tables rounded to float (fp32 launches)
     int32_t *d_pint = nullptr /* 5*npairs: bfa,bfb,sha,shb,knom */;
     double *d_boysp = nullptr;                // per-order Taylor tables [BOYS_MORD][BOYS_NT][BOYS_NC] (generated kernels)
     PairTable tab{};
@@ -238,11 +275,11 @@ struct adft_shellpairs {
     size_t segs_cap = 0;
     unsigned long long *d_counters = nullptr, *d_dmax = nullptr, *h_small = nullptr;
     int32_t *d_prim_err = nullptr;     // raised by pair_prim_kernel when a pair's survivor count is not its sublist's K
-    cudaEvent_t ev[2 * NQCLASS + 8] = {};
+    cudaEvent_t ev[4 * NQCLASS + 8] = {};      // [0,2N) fp64 class launches, [2N,2N+8) phases, [2N+8,4N+8) fp32 class launches
     bool ev_ok = false;
     // last build
     adft_jk_stats_t stats{};
-    bool class_ran[NQCLASS] = {};
+    bool class_ran[NQCLASS] = {}, class_ran32[NQCLASS] = {};
     bool have_build = false;
     cudaStream_t last_stream = nullptr;
     // staging for adft_jk_build_host
@@ -250,6 +287,9 @@ struct adft_shellpairs {
     size_t stage_n = 0;
     double *d_rys = nullptr;                  // device copy of the Rys tables
     RysTable rys{};
+    int32_t *d_bfoff = nullptr;               // [nshells+1] first basis function of every shell
+    double *d_dsh = nullptr;                  // [nshells*nshells] |D|_XY of the block-density screen (R-23)
+    double *d_incr = nullptr;                 // 3 N^2 scratch of adft_jk_build_incremental: dD, J(dD), K(dD)
 };
 
 // ------------------------------------------------------------------ misc API
@@ -382,7 +422,8 @@ static void free_pairs(adft_shellpairs *p)
     cudaFree(p->d_xyz); cudaFree(p->d_expo); cudaFree(p->d_coef); cudaFree(p->d_atom); cudaFree(p->d_nprim);
     cudaFree(p->d_off); cudaFree(p->d_Q); cudaFree(p->d_AB); cudaFree(p->d_prim); cudaFree(p->d_pint);
     cudaFree(p->d_boysp); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage);
-    cudaFree(p->d_rys); cudaFree(p->d_prim_err);
+    cudaFree(p->d_rys); cudaFree(p->d_prim_err); cudaFree(p->d_bfoff); cudaFree(p->d_dsh); cudaFree(p->d_incr);
+    cudaFree(p->d_primf); cudaFree(p->d_boysf);
     if (p->h_segs) cudaFreeHost(p->h_segs);
     if (p->h_small) cudaFreeHost(p->h_small);
     if (p->ev_ok) for (auto &e : p->ev) cudaEventDestroy(e);
@@ -403,6 +444,8 @@ static void set_table_pointers(adft_shellpairs *p)
     t.zeta = p->d_prim; t.inv2z = p->d_prim + npp; t.Px = p->d_prim + 2 * npp; t.Py = p->d_prim + 3 * npp;
     t.Pz = p->d_prim + 4 * npp; t.PAx = p->d_prim + 5 * npp; t.PAy = p->d_prim + 6 * npp; t.PAz = p->d_prim + 7 * npp;
     t.cc = p->d_prim + 8 * npp;
+    t.zeta_f = p->d_primf; t.inv2z_f = p->d_primf + npp; t.PAx_f = p->d_primf + 2 * npp; t.PAy_f = p->d_primf + 3 * npp;
+    t.PAz_f = p->d_primf + 4 * npp; t.cc_f = p->d_primf + 5 * npp;
 }
 
 static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vector<HostPair> &hp, double thr, cudaStream_t st)
@@ -429,7 +472,7 @@ static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vecto
                                                              p->d_prim_err, p->tab.sha, p->tab.shb, p->d_atom,
                                                              p->d_nprim, p->d_off, p->d_xyz, p->d_expo, p->d_coef, f, f + npp,
                                                              f + 2 * npp, f + 3 * npp, f + 4 * npp, f + 5 * npp, f + 6 * npp,
-                                                             f + 7 * npp, f + 8 * npp);
+                                                             f + 7 * npp, f + 8 * npp, p->d_primf, npp);
     }
     CUDA_TRY(cudaGetLastError());
     int32_t bad = 0;
@@ -549,11 +592,15 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     ALLOC(p->d_AB, 3 * np * sizeof(double));
     ALLOC(p->d_pint, 5 * np * sizeof(int32_t));
     ALLOC(p->d_prim, 9 * npp * sizeof(double));
+    ALLOC(p->d_primf, 6 * npp * sizeof(float));
+    ALLOC(p->d_boysf, (size_t)BOYS_MORD * BOYS_NT * BOYS_NC * sizeof(float));
     ALLOC(p->d_boysp, (size_t)BOYS_MORD * BOYS_NT * BOYS_NC * sizeof(double));
-    ALLOC(p->d_counters, 4 * NQCLASS * sizeof(unsigned long long));
+    ALLOC(p->d_counters, 8 * NQCLASS * sizeof(unsigned long long));     // [0,4N) all launches' fp64 part, [4N,8N) fp32 launches
     ALLOC(p->d_dmax, 2 * sizeof(unsigned long long));
     ALLOC(p->d_prim_err, sizeof(int32_t));
     ALLOC(p->d_rys, (size_t)(adft_rys_blob_end - adft_rys_blob) * sizeof(double));
+    ALLOC(p->d_bfoff, (ns + 1) * sizeof(int32_t));
+    ALLOC(p->d_dsh, (size_t)ns * ns * sizeof(double));
 #undef ALLOC
     {
         // Rys tables (gen_rys.py layout): header[8] = magic, NMAX, TMAX, H, NCOEF
@@ -567,7 +614,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
         for (int n = 1; n <= 7; ++n) { p->rys.off_asym[n] = off; off += 2 * n; }
         if (off != (int)(adft_rys_blob_end - adft_rys_blob)) { set_error("adft_shellpairs_build: Rys table size mismatch"); free_pairs(p); return ADFT_ERR_INTERNAL; }
     }
-    if (cudaMallocHost((void **)&p->h_small, 4 * NQCLASS * sizeof(unsigned long long)) != cudaSuccess) {
+    if (cudaMallocHost((void **)&p->h_small, 8 * NQCLASS * sizeof(unsigned long long)) != cudaSuccess) {
         set_error("adft_shellpairs_build: cudaMallocHost failed"); free_pairs(p); return ADFT_ERR_ALLOC;
     }
     for (auto &e : p->ev)
@@ -591,6 +638,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     TRY2(cudaMemcpyAsync(p->d_atom, b->atom.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     TRY2(cudaMemcpyAsync(p->d_nprim, b->nprimv.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     TRY2(cudaMemcpyAsync(p->d_off, b->off.data(), ns * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    TRY2(cudaMemcpyAsync(p->d_bfoff, b->bf_off.data(), (ns + 1) * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     TRY2(cudaMemcpyAsync(p->d_rys, adft_rys_blob, (size_t)(adft_rys_blob_end - adft_rys_blob) * sizeof(double),
                          cudaMemcpyHostToDevice, st));
     std::vector<double> boys;
@@ -606,6 +654,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
             }
         }
     TRY2(cudaMemcpyAsync(p->d_boysp, boysp.data(), boysp.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    std::vector<float> boysf(boysp.begin(), boysp.end());
+    TRY2(cudaMemcpyAsync(p->d_boysf, boysf.data(), boysf.size() * sizeof(float), cudaMemcpyHostToDevice, st));
     TRY2(cudaStreamSynchronize(st));
 
     // pass 1: records of ALL primitive pairs in bucket order, Schwarz bounds from the full contraction
@@ -631,7 +681,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
             pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.K, s.la, s.lb, prim_threshold,
                                                                  d_kcount, p->d_prim_err, p->tab.sha, p->tab.shb, p->d_atom, p->d_nprim,
                                                                  p->d_off, p->d_xyz, p->d_expo, p->d_coef, nullptr, nullptr,
-                                                                 nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                 nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+                                                                 nullptr, 0);
         }
         TRY2(cudaGetLastError());
         std::vector<int32_t> kc(np);
@@ -648,6 +699,9 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
             TRY2(cudaFree(p->d_prim));
             p->d_prim = nullptr;
             TRY2(cudaMalloc((void **)&p->d_prim, 9 * (size_t)p->nprimpairs * sizeof(double)));
+            TRY2(cudaFree(p->d_primf));
+            p->d_primf = nullptr;
+            TRY2(cudaMalloc((void **)&p->d_primf, 6 * (size_t)p->nprimpairs * sizeof(float)));
         }
         set_table_pointers(p);
     }
@@ -706,7 +760,11 @@ static int prefix_len(const double *q, int n, double qfix, double dmax, double t
     return lo;
 }
 
-static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax, double tau, std::vector<Segment> &segs)
+// tau_skip > 0 (the fp32 launch of the mixed-precision dispatch, global-Dmax rule only): tile columns that lie, for EVERY
+// row of the segment, inside the fp64 prefix (S >= tau_skip) are left out of the launch.  The last row has the smallest
+// Q_ab and therefore the shortest fp64 prefix; columns below it are fp64 for all rows.
+static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax, double tau, std::vector<Segment> &segs,
+                            double tau_skip = 0.0)
 {
     segs.clear();
     for (int i1 : p->subl_of_class[X])
@@ -724,6 +782,11 @@ static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax,
             sg.bra_pair_base = s1.pair_base; sg.bra_prim_base = s1.prim_base; sg.bra_n = s1.n; sg.bra_K = s1.K;
             sg.ket_pair_base = s2.pair_base; sg.ket_prim_base = s2.prim_base; sg.ket_n = s2.n; sg.ket_K = s2.K;
             sg.rows = rows; sg.tiles_per_row = (cols + TILE_C - 1) / TILE_C; sg.same = same ? 1 : 0;
+            if (tau_skip > 0.0) {
+                sg.col_tile_begin = prefix_len(q2, s2.n, q1[rows - 1], dmax, tau_skip) / TILE_C;
+                sg.tiles_per_row -= sg.col_tile_begin;
+                if (sg.tiles_per_row <= 0) continue;
+            }
             segs.push_back(sg);
         }
     // heaviest tiles first (per-tile cost ~ K1*K2), so the tail of the launch is made of cheap tiles
@@ -739,7 +802,27 @@ static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax,
 extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, double *J, double *K, double tau,
                                        void *cuda_stream)
 {
+    return adft_jk_build_ex(p, D, J, K, tau, nullptr, cuda_stream);
+}
+
+extern "C" adft_status_t adft_jk_build_ex(adft_shellpairs_t *p, const double *D, double *J, double *K, double tau,
+                                          const adft_jk_options_t *opt, void *cuda_stream)
+{
     if (!p || !D || (!J && !K)) { set_error("adft_jk_build: NULL handle or D, or both J and K NULL"); return ADFT_ERR_INVALID_ARG; }
+    const uint32_t flags = opt ? opt->flags : 0u;
+    const int shard_count = opt && opt->shard_count > 1 ? opt->shard_count : 1;
+    const int shard_rank = opt ? opt->shard_rank : 0;
+    if (flags & ~(ADFT_JK_BLOCK_DENSITY | ADFT_JK_MIXED_PRECISION)) { set_error("adft_jk_build_ex: unknown option flags"); return ADFT_ERR_INVALID_ARG; }
+    const bool mixed = (flags & ADFT_JK_MIXED_PRECISION) != 0;
+    const double band = opt && opt->fp32_band != 0.0 ? opt->fp32_band : ADFT_DEFAULT_FP32_BAND;
+    if (mixed && (!J || !K)) { set_error("adft_jk_build_ex: ADFT_JK_MIXED_PRECISION needs both J and K"); return ADFT_ERR_INVALID_ARG; }
+    if (mixed && (!(band >= 1.0) || !std::isfinite(band))) { set_error("adft_jk_build_ex: fp32_band must be finite and >= 1"); return ADFT_ERR_INVALID_ARG; }
+    const double tau64 = tau * band;          // S >= tau64: double precision; tau <= S < tau64: single precision
+    if (opt && (opt->shard_count < 0 || shard_rank < 0 || shard_rank >= shard_count)) {
+        set_error("adft_jk_build_ex: shard_rank must lie in [0, shard_count)");
+        return ADFT_ERR_INVALID_ARG;
+    }
+    const bool block_density = (flags & ADFT_JK_BLOCK_DENSITY) != 0;
     if (!(tau >= 0.0) || !std::isfinite(tau)) { set_error("adft_jk_build: schwarz_threshold must be finite and >= 0"); return ADFT_ERR_INVALID_ARG; }
     if (D == J || D == K || J == K) { set_error("adft_jk_build: D, J and K must not alias one another"); return ADFT_ERR_INVALID_ARG; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -767,16 +850,29 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
     if (p->h_small[1]) { set_error("adft_jk_build: D contains NaN or Inf"); return ADFT_ERR_NOT_FINITE; }
     double dmax;
     std::memcpy(&dmax, &p->h_small[0], sizeof(double));
+    if (block_density) {
+        // (f3) shell-block maxima of |D|; the host plan below still bounds the rectangles with the global Dmax (a
+        // superset of what the block rule keeps), the exact rule is applied per lane
+        const int ns = p->basis->nshells;
+        const long long nn = (long long)ns * ns;
+        dshell_kernel<<<(unsigned)((nn + 255) / 256), 256, 0, st>>>(D, N, p->d_bfoff, ns, p->d_dsh); ++launches;
+        CUDA_TRY(cudaGetLastError());
+    }
 
     // plan: segments of every class
-    std::vector<std::vector<Segment>> plan(NQCLASS);
-    long long warps[NQCLASS] = {};
+    // (f1, mixed precision) the straight-line classes get two launches: the fp64 kernel over the rectangles of the rule
+    // S >= tau64 and the fp32 kernel over those of S >= tau minus the leading all-fp64 columns; each lane applies the exact
+    // band test, so every kept quartet is evaluated exactly once.  The Rys classes (f shells) stay fp64 throughout.
+    std::vector<std::vector<Segment>> plan(NQCLASS), plan32(NQCLASS);
+    long long warps[NQCLASS] = {}, warps32[NQCLASS] = {};
     size_t nseg_total = 0;
     for (int X = 0; X < NPAIRCLASS; ++X)
         for (int Y = 0; Y <= X; ++Y) {
             const int qc = quartet_class(X, Y);
-            warps[qc] = plan_class(p, X, Y, dmax, tau, plan[qc]);
-            nseg_total += plan[qc].size();
+            const bool two = mixed && tau > 0.0 && !class_table()[qc].use_rys;
+            warps[qc] = plan_class(p, X, Y, dmax, two ? tau64 : tau, plan[qc]);
+            if (two) warps32[qc] = plan_class(p, X, Y, dmax, tau, plan32[qc], block_density ? 0.0 : tau64);
+            nseg_total += plan[qc].size() + plan32[qc].size();
         }
     if (nseg_total > p->segs_cap) {
         cudaFree(p->d_segs); if (p->h_segs) cudaFreeHost(p->h_segs);
@@ -786,17 +882,20 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
         CUDA_TRY(cudaMallocHost((void **)&p->h_segs, cap * sizeof(Segment)));
         p->segs_cap = cap;
     }
-    size_t seg_off[NQCLASS] = {};
+    size_t seg_off[NQCLASS] = {}, seg_off32[NQCLASS] = {};
     {
         size_t o = 0;
         for (int qc = 0; qc < NQCLASS; ++qc) {
             seg_off[qc] = o;
             std::copy(plan[qc].begin(), plan[qc].end(), p->h_segs + o);
             o += plan[qc].size();
+            seg_off32[qc] = o;
+            std::copy(plan32[qc].begin(), plan32[qc].end(), p->h_segs + o);
+            o += plan32[qc].size();
         }
         if (o) CUDA_TRY(cudaMemcpyAsync(p->d_segs, p->h_segs, o * sizeof(Segment), cudaMemcpyHostToDevice, st));
     }
-    CUDA_TRY(cudaMemsetAsync(p->d_counters, 0, 4 * NQCLASS * sizeof(unsigned long long), st));
+    CUDA_TRY(cudaMemsetAsync(p->d_counters, 0, 8 * NQCLASS * sizeof(unsigned long long), st));
     if (J) CUDA_TRY(cudaMemsetAsync(J, 0, n2 * sizeof(double), st));
     if (K) CUDA_TRY(cudaMemsetAsync(K, 0, n2 * sizeof(double), st));
     CUDA_TRY(cudaEventRecord(ev_plan, st));
@@ -807,22 +906,40 @@ extern "C" adft_status_t adft_jk_build(adft_shellpairs_t *p, const double *D, do
     std::stable_sort(order, order + NQCLASS, [&](int a, int b) { return a > b; });
     for (int qi = 0; qi < NQCLASS; ++qi) {
         const int qc = order[qi];
-        p->class_ran[qc] = false;
-        if (warps[qc] == 0) continue;
+        p->class_ran[qc] = p->class_ran32[qc] = false;
+        if (warps[qc] == 0 && warps32[qc] == 0) continue;
+        const ClassEntry &ce = class_table()[qc];
+        const bool two = mixed && tau > 0.0 && !ce.use_rys;
         JKParams prm{};
         prm.t = p->tab; prm.segs = p->d_segs + seg_off[qc]; prm.nsegs = (int)plan[qc].size(); prm.total_warps = warps[qc];
-        prm.D = D; prm.J = J; prm.K = K; prm.N = N; prm.tau = tau; prm.dmax = dmax; prm.boys = p->d_boysp;
+        prm.D = D; prm.J = J; prm.K = K; prm.N = N; prm.tau = two ? tau64 : tau; prm.tau_hi = HUGE_VAL; prm.dmax = dmax;
+        prm.boys = p->d_boysp; prm.boys_f = p->d_boysf;
         prm.counters = p->d_counters + 4 * qc; prm.zero = 0;
-        CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
-        const ClassEntry &ce = class_table()[qc];
-        if (ce.use_rys) {
-            CUDA_TRY(rys_jk_launcher(ce.la, ce.lb, ce.lc, ce.ld)(prm, p->rys, p->d_counters + 4 * qc + 3, st, J != nullptr, K != nullptr));
-        } else {
-            ce.launch_jk(prm, st, J != nullptr, K != nullptr);
+        prm.Dsh = block_density ? p->d_dsh : nullptr; prm.nshells = p->basis->nshells;
+        prm.shard_rank = shard_rank; prm.shard_count = shard_count;
+        if (warps[qc] > 0) {
+            CUDA_TRY(cudaEventRecord(ev[2 * qc], st));
+            if (ce.use_rys) {
+                CUDA_TRY(rys_jk_launcher(ce.la, ce.lb, ce.lc, ce.ld)(prm, p->rys, p->d_counters + 4 * qc + 3, st, J != nullptr, K != nullptr));
+            } else {
+                ce.launch_jk(prm, st, J != nullptr, K != nullptr, false);
+            }
+            ++launches;
+            CUDA_TRY(cudaEventRecord(ev[2 * qc + 1], st));
+            p->class_ran[qc] = true;
         }
-        ++launches;
-        CUDA_TRY(cudaEventRecord(ev[2 * qc + 1], st));
-        p->class_ran[qc] = true;
+        if (two && warps32[qc] > 0) {
+            // the single-precision band tau <= S < tau64 of this class
+            prm.segs = p->d_segs + seg_off32[qc]; prm.nsegs = (int)plan32[qc].size(); prm.total_warps = warps32[qc];
+            prm.tau = tau; prm.tau_hi = tau64;
+            prm.counters = p->d_counters + 4 * NQCLASS + 4 * qc;
+            cudaEvent_t *e32 = ev + 2 * NQCLASS + 8;
+            CUDA_TRY(cudaEventRecord(e32[2 * qc], st));
+            ce.launch_jk(prm, st, true, true, true);
+            ++launches;
+            CUDA_TRY(cudaEventRecord(e32[2 * qc + 1], st));
+            p->class_ran32[qc] = true;
+        }
     }
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaEventRecord(ev_eri, st));
@@ -846,18 +963,21 @@ extern "C" adft_status_t adft_jk_stats(adft_shellpairs_t *p, adft_jk_stats_t *ou
     if (!p || !out) { set_error("adft_jk_stats: NULL"); return ADFT_ERR_INVALID_ARG; }
     if (!p->have_build) { set_error("adft_jk_stats: no build yet"); return ADFT_ERR_INVALID_ARG; }
     cudaStream_t st = p->last_stream;
-    CUDA_TRY(cudaMemcpyAsync(p->h_small, p->d_counters, 4 * NQCLASS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(p->h_small, p->d_counters, 8 * NQCLASS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     adft_jk_stats_t &s = p->stats;
     cudaEvent_t *ev = p->ev;
-    s.quartets_kept = 0; s.prim_quartets = 0; s.prim_quartets_evaluated = 0; s.model_flops = 0.0;
+    s.quartets_kept = 0; s.prim_quartets = 0; s.prim_quartets_evaluated = 0; s.model_flops = 0.0; s.quartets_fp32 = 0;
     for (int qc = 0; qc < NQCLASS; ++qc) {
-        s.class_quartets[qc] = (int64_t)p->h_small[4 * qc];
-        const int64_t prim = (int64_t)p->h_small[4 * qc + 1];       // evaluated (after primitive screening)
+        const unsigned long long *c32 = p->h_small + 4 * NQCLASS + 4 * qc;      // the fp32 launch of this class
+        s.class_quartets_fp32[qc] = (int64_t)c32[0];
+        s.quartets_fp32 += (int64_t)c32[0];
+        s.class_quartets[qc] = (int64_t)(p->h_small[4 * qc] + c32[0]);
+        const int64_t prim = (int64_t)(p->h_small[4 * qc + 1] + c32[1]);       // evaluated (after primitive screening)
         s.quartets_kept += s.class_quartets[qc];
         s.prim_quartets_evaluated += prim;
         s.class_prim_quartets[qc] = prim;
-        s.prim_quartets += (int64_t)p->h_small[4 * qc + 2];
+        s.prim_quartets += (int64_t)(p->h_small[4 * qc + 2] + c32[2]);
         const ClassEntry &ce = class_table()[qc];
         const int L = ce.la + ce.lb + ce.lc + ce.ld;
         // model flops: per primitive quartet 60+4L (geometry, prefactor, Boys) + generated VRR instructions
@@ -868,6 +988,9 @@ extern "C" adft_status_t adft_jk_stats(adft_shellpairs_t *p, adft_jk_stats_t *ou
         float ms = 0.f;
         s.class_ms[qc] = 0.0;
         if (p->class_ran[qc] && cudaEventElapsedTime(&ms, ev[2 * qc], ev[2 * qc + 1]) == cudaSuccess) s.class_ms[qc] = ms;
+        s.class_ms_fp32[qc] = 0.0;
+        if (p->class_ran32[qc] && cudaEventElapsedTime(&ms, ev[2 * NQCLASS + 8 + 2 * qc], ev[2 * NQCLASS + 8 + 2 * qc + 1]) == cudaSuccess)
+            s.class_ms_fp32[qc] = ms;
     }
     float ms = 0.f;
     const int B = 2 * NQCLASS;
@@ -878,6 +1001,29 @@ extern "C" adft_status_t adft_jk_stats(adft_shellpairs_t *p, adft_jk_stats_t *ou
     if (cudaEventElapsedTime(&ms, ev[B], ev[B + 4]) == cudaSuccess) s.ms_total = ms;
     cudaGetLastError();
     *out = s;
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_jk_build_incremental(adft_shellpairs_t *p, const double *D, double *Dprev, double *J, double *K,
+                                                   double tau, const adft_jk_options_t *opt, void *cuda_stream)
+{
+    if (!p || !D || !Dprev || (!J && !K)) { set_error("adft_jk_build_incremental: NULL handle, D or D_prev, or both J and K NULL"); return ADFT_ERR_INVALID_ARG; }
+    if (Dprev == D || Dprev == J || Dprev == K) { set_error("adft_jk_build_incremental: D_prev must not alias D, J or K"); return ADFT_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n2 = (size_t)p->basis->nbf * p->basis->nbf;
+    if (!p->d_incr) CUDA_TRY(cudaMalloc((void **)&p->d_incr, 3 * n2 * sizeof(double)));
+    double *dD = p->d_incr, *Js = J ? p->d_incr + n2 : nullptr, *Ks = K ? p->d_incr + 2 * n2 : nullptr;
+    const unsigned nb = (unsigned)std::min<size_t>((n2 + 255) / 256, (size_t)p->sm_count * 8);
+    diff_kernel<<<nb, 256, 0, st>>>(D, Dprev, dD, n2);
+    CUDA_TRY(cudaGetLastError());
+    adft_jk_options_t o{};
+    if (opt) o = *opt;
+    o.flags |= ADFT_JK_BLOCK_DENSITY;
+    adft_status_t rc = adft_jk_build_ex(p, dD, Js, Ks, tau, &o, cuda_stream);
+    if (rc) return rc;
+    incr_finish_kernel<<<nb, 256, 0, st>>>(J, Js, K, Ks, Dprev, D, n2);
+    CUDA_TRY(cudaGetLastError());
+    p->stats.kernel_launches += 2;
     return ADFT_OK;
 }
 

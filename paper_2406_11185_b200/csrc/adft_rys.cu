@@ -32,7 +32,8 @@ template <class C, bool WJ, bool WK>
 static cudaError_t run_jk_variant(const JKParams &p, const RysTable &rt, unsigned long long *tile_counter, cudaStream_t st)
 {
     const int nblocks = resident_blocks<C, WJ, WK>();
-    const long long want = p.total_warps;
+    const long long want = (p.total_warps - p.shard_rank + p.shard_count - 1) / p.shard_count;      // tiles of this rank
+    if (want <= 0) return cudaSuccess;
     return launch_jk_rys<C, WJ, WK>(p, rt, tile_counter, (int)(want < nblocks ? want : nblocks), st);
 }
 

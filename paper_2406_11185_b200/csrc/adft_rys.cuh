@@ -409,7 +409,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p
     for (;;) {
         if (tid == 0) s_tile = (long long)atomicAdd(tile_counter, 1ull);
         __syncthreads();
-        const long long w = s_tile;
+        const long long w = s_tile * p.shard_count + p.shard_rank;
         __syncthreads();
         if (w >= p.total_warps) break;
         int lo = 0, hi = p.nsegs - 1;
@@ -419,25 +419,27 @@ __global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p
         }
         const Segment sg = p.segs[lo];
         const long long r = w - sg.warp_begin;
-        const int i_base = (int)(r / sg.tiles_per_row) * TILE_R, j_base = (int)(r % sg.tiles_per_row) * TILE_C;
+        const int i_base = (int)(r / sg.tiles_per_row) * TILE_R, j_base = ((int)(r % sg.tiles_per_row) + sg.col_tile_begin) * TILE_C;
         for (int jj = 0; jj < 32; ++jj) {                       // the 32 quartets of the tile, one after the other
             const int i = i_base + jj / TILE_C, j = j_base + (jj & (TILE_C - 1));
             if (i >= sg.rows) break;
             if (j >= (sg.same ? (i + 1) : sg.ket_n)) continue;
             const int gab = sg.bra_pair_base + i, gcd = sg.ket_pair_base + j;
-            if (!((__ldg(p.t.Q + gab) * __ldg(p.t.Q + gcd)) * p.dmax >= p.tau)) continue;   // the screen (DESIGN R-7)
+            // the screen (DESIGN R-7; block-density rule R-23 when p.Dsh is set)
+            const double S = (__ldg(p.t.Q + gab) * __ldg(p.t.Q + gcd)) * screen_density(p, gab, gcd);
+            if (!(S >= p.tau && S < p.tau_hi)) continue;
             if (tid == 0) {
                 cnt_q += 1ull;
                 cnt_p += (unsigned long long)(sg.bra_K * sg.ket_K);
                 cnt_n += (unsigned long long)((unsigned)__ldg(p.t.knom + gab) * (unsigned)__ldg(p.t.knom + gcd));
             }
-            const int sa = __ldg(p.t.sha + gab), sb = __ldg(p.t.shb + gab);
             const int a0 = __ldg(p.t.bfa + gab), b0 = __ldg(p.t.bfb + gab);
             const double AB[3] = {__ldg(p.t.ABx + gab), __ldg(p.t.ABy + gab), __ldg(p.t.ABz + gab)};
             const double CD[3] = {__ldg(p.t.ABx + gcd), __ldg(p.t.ABy + gcd), __ldg(p.t.ABz + gcd)};
             double acc[C::CH];
             rys_quartet<C>(p.t, rt, sm, sg.bra_prim_base + i, sg.bra_n, sg.bra_K, sg.ket_prim_base + j, sg.ket_n, sg.ket_K,
                            AB, CD, chunk, offx, offy, offz, acc);
+            const int sa = __ldg(p.t.sha + gab), sb = __ldg(p.t.shb + gab);
             const int sc = __ldg(p.t.sha + gcd), sd = __ldg(p.t.shb + gcd);
             double wgt = 1.0;
             if (sa == sb) wgt *= 0.5;

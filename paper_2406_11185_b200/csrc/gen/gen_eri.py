@@ -178,25 +178,25 @@ class VrrDag:
                 if s[7]:
                     used_ze.add(s[6])
         for n in sorted(used_z):
-            out.append(f"    const double kz{n} = {float(n)} * c.inv2z;")
+            out.append(f"    const R kz{n} = R({float(n)}) * c.inv2z;")
         for n in sorted(used_e):
-            out.append(f"    const double ke{n} = {float(n)} * c.inv2e;")
+            out.append(f"    const R ke{n} = R({float(n)}) * c.inv2e;")
         for n in sorted(used_ze):
-            out.append(f"    const double kx{n} = {float(n)} * c.inv2ze;")
+            out.append(f"    const R kx{n} = R({float(n)}) * c.inv2ze;")
         tgt_index = {("V", a, cc, 0): j for j, (a, cc) in enumerate(self.targets)}
         for key, s in self.nodes.items():
             v = name(key)
             if s[0] == "B":
-                out.append(f"    const double {v} = F[{s[1]}];")
+                out.append(f"    const R {v} = F[{s[1]}];")
             elif s[0] == "T":
                 r = "c.roz" if s[1] == "bra" else "c.roe"
-                out.append(f"    const double {v} = fma(-{r}, {name(s[3])}, {name(s[2])});")
+                out.append(f"    const R {v} = fma(-{r}, {name(s[3])}, {name(s[2])});")
             elif s[0] == "A":
                 _, i, d0, d1, n2, t2 = s
                 e = f"fma(c.PA{AX[i]}, {name(d0)}, c.WP{AX[i]} * {name(d1)})"
                 if t2:
                     e = f"fma(kz{n2}, {name(t2)}, {e})"
-                out.append(f"    const double {v} = {e};")
+                out.append(f"    const R {v} = {e};")
             else:
                 _, i, d0, d1, n2, t2, nx, tx = s
                 e = f"fma(c.QC{AX[i]}, {name(d0)}, c.WQ{AX[i]} * {name(d1)})"
@@ -204,7 +204,7 @@ class VrrDag:
                     e = f"fma(ke{n2}, {name(t2)}, {e})"
                 if tx:
                     e = f"fma(kx{nx}, {name(tx)}, {e})"
-                out.append(f"    const double {v} = {e};")
+                out.append(f"    const R {v} = {e};")
             if key in tgt_index:
                 out.append(f"    acc.template add<{tgt_index[key]}>({v});")
 
@@ -299,7 +299,7 @@ class HrrDag:
                 emit_node(s[1]); emitted.add(k); return
             _, which, i, k0, k1 = s
             emit_node(k0); emit_node(k1)
-            out.append(f"    const double h{self.ids[k]} = fma({which}{AX[i]}, {name(k1)}, {name(k0)});")
+            out.append(f"    const R h{self.ids[k]} = fma({which}{AX[i]}, {name(k1)}, {name(k0)});")
             emitted.add(k)
 
         for (ia, ib, ic, idd, k) in self.outputs:
@@ -361,13 +361,13 @@ def generate_class(la, lb, lc, ld, cmax_list=()):
     o.append(f"    static constexpr int NA = {ncart(la)}, NB = {ncart(lb)}, NC = {ncart(lc)}, ND = {ncart(ld)};")
     o.append(f"    static constexpr int NE = {NE}, NF = {NF}, NACC = {NE * NF}, MMAX = {vrr.max_m()};")
     o.append(f"    static constexpr int VRR_OPS = {vrr.fp64_ops()}, HRR_OPS = {hrr.fp64_ops()}, NINT = {nint};")
-    o.append("    template <class Ctx, class Acc>")
-    o.append("    static __device__ __forceinline__ void vrr(const Ctx &c, const double *__restrict__ F, Acc &acc) {")
+    o.append("    // R = the arithmetic type (double, or float for the single-precision band of the mixed-precision dispatch)")
+    o.append("    template <class Ctx, class Acc, class R>")
+    o.append("    static __device__ __forceinline__ void vrr(const Ctx &c, const R *__restrict__ F, Acc &acc) {")
     vrr.emit(o)
     o.append("    }")
-    o.append("    template <class Acc, class Dg>")
-    o.append("    static __device__ __forceinline__ void hrr(const Acc &acc, double ABx, double ABy, double ABz,")
-    o.append("                                                double CDx, double CDy, double CDz, Dg &dg) {")
+    o.append("    template <class Acc, class Dg, class R>")
+    o.append("    static __device__ __forceinline__ void hrr(const Acc &acc, R ABx, R ABy, R ABz, R CDx, R CDy, R CDz, Dg &dg) {")
     hrr.emit(o)
     o.append("    }")
     o.append("};")
@@ -385,8 +385,8 @@ def generate_class(la, lb, lc, ld, cmax_list=()):
         o.append(f"    static constexpr int NCHUNK_MAX = {max(len(p.targets) for p in passes)};")
         o.append("    static __host__ __device__ constexpr int pass_nacc(int P) { constexpr int t[] = {" + ", ".join(str(len(p.targets)) for p in passes) + "}; return t[P]; }")
         o.append("    static __host__ __device__ constexpr int pass_mmax(int P) { constexpr int t[] = {" + ", ".join(str(p.max_m()) for p in passes) + "}; return t[P]; }")
-        o.append("    template <int P, class Ctx, class Acc>")
-        o.append("    static __device__ __forceinline__ void vrr_pass(const Ctx &c, const double *__restrict__ F, Acc &acc) {")
+        o.append("    template <int P, class Ctx, class Acc, class R>")
+        o.append("    static __device__ __forceinline__ void vrr_pass(const Ctx &c, const R *__restrict__ F, Acc &acc) {")
         for k, pdag in enumerate(passes):
             o.append(f"      if constexpr (P == {k}) {{")
             pdag.emit(o)

@@ -190,3 +190,33 @@ def make_custom(atoms, shell_specs, seed, tau=0.0, nocc=None, emin=0.1, emax=50.
     return Workload("custom", atoms, np.array(s_atom, np.int32), np.array(s_l, np.int32),
                     np.array(s_np, np.int32), np.array(s_off, np.int32),
                     np.array(exps, np.float64), np.array(cofs, np.float64), D, tau)
+
+
+def sparse_density(w, seed, decades=8.0):
+    """Input generator of the block-density tests: the workload's D with every shell block scaled by its
+    own factor 10^-U(0, decades) (symmetric), so that the block maxima |D|_XY spread over `decades` orders of magnitude
+    the way a density difference between two SCF iterations does.  No method arithmetic."""
+    rng = np.random.default_rng(seed)
+    o = w.bf_offsets()
+    f = 10.0 ** (-decades * rng.random((w.nshells, w.nshells)))
+    f = np.minimum(f, f.T)
+    D = np.array(w.D)
+    for X in range(w.nshells):
+        for Y in range(w.nshells):
+            D[o[X]:o[X + 1], o[Y]:o[Y + 1]] *= f[X, Y]
+    return np.ascontiguousarray((D + D.T) / 2)
+
+
+def perturbed_density(w, seed, atoms=(0,), scale=1e-3):
+    """Input generator of the incremental-build tests: D plus a symmetric perturbation of relative size `scale` confined
+    to the rows and columns of the basis functions on the given atoms (what one SCF step changes near a site)."""
+    rng = np.random.default_rng(seed)
+    o = w.bf_offsets()
+    on = np.zeros(w.nbf, bool)
+    for s in range(w.nshells):
+        if int(w.shell_atom[s]) in atoms:
+            on[o[s]:o[s + 1]] = True
+    P = rng.normal(size=(w.nbf, w.nbf)) * scale * np.abs(w.D).max()
+    P = (P + P.T) / 2
+    P[~(on[:, None] | on[None, :])] = 0.0
+    return np.ascontiguousarray(np.array(w.D) + P)

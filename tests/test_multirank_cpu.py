@@ -44,6 +44,56 @@ def test_max_over_ranks_and_job_value_world2():
         assert v == pytest.approx(2 * 1000 / 0.125)              # two replicas in the time of the slower one
 
 
+def _shard_worker(rank, world, port, out):
+    """One rank of the sharded build's host path on CPU: shard_of() -> (rank, world); a partial J, K (here from the
+    oracle's loop over this rank's share of the bra pairs; on a GPU from adft_jk_build_ex with shard_rank/shard_count);
+    allreduce_jk() sums them in place over the group."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import oracle
+    from paper_2406_11185_b200 import api, workloads as W
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    assert api.shard_of() == (rank, world)
+    w = W.make("0b")
+    bs = oracle.basis_from_workload(w)
+    Q = oracle.schwarz(bs)
+    npair = bs.nshells * (bs.nshells + 1) // 2
+    lo, hi = rank * npair // world, (rank + 1) * npair // world
+    Jp, Kp, cnt = oracle.jk_range(bs, w.D, w.tau, Q, lo, hi)
+    J = torch.from_numpy(np.asarray(Jp, np.float64)); K = torch.from_numpy(np.asarray(Kp, np.float64))
+    api.allreduce_jk(J, K)
+    api.allreduce_jk(J.clone(), None)                   # a J-only build reduces one matrix
+    out[rank] = (J.numpy().copy(), K.numpy().copy(), cnt["kept"])
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_sharded_build_allreduce_world2():
+    import numpy as np
+    import torch.multiprocessing as mp
+    import oracle
+    from paper_2406_11185_b200 import workloads as W
+    port = _free_port()
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_shard_worker, args=(2, port, out), nprocs=2, join=True)
+        res = dict(out)
+    w = W.make("0b")
+    bs = oracle.basis_from_workload(w)
+    Jo, Ko, cnt = oracle.jk(bs, w.D, w.tau)
+    assert res[0][2] + res[1][2] == cnt["kept"] and res[0][2] > 0 and res[1][2] > 0
+    for r in (0, 1):                                     # every rank ends with the full matrices
+        assert np.abs(res[r][0] - Jo).max() <= 1e-12 and np.abs(res[r][1] - Ko).max() <= 1e-12
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+
+
+def test_shard_of_without_process_group():
+    from paper_2406_11185_b200 import api
+    assert api.shard_of() == (0, 1)
+    api.allreduce_jk(None, None)                         # no group: nothing to do
+
+
 def test_world1_is_identity():
     import bench
     assert bench.reduce_max_over_ranks([3.5, 7.25], 1) == [3.5, 7.25]

@@ -21,18 +21,7 @@ def _dshell_numpy(bs, D):
     return out
 
 
-def _sparse_density(w, seed, decades=8.0):
-    """The workload's D with shell blocks scaled by widely different factors (symmetric), so that the block maxima
-    spread over `decades` orders of magnitude and the block rule differs from the global one."""
-    rng = np.random.default_rng(seed)
-    o = w.bf_offsets()
-    f = 10.0 ** (-decades * rng.random((w.nshells, w.nshells)))
-    f = np.minimum(f, f.T)
-    D = np.array(w.D)
-    for X in range(w.nshells):
-        for Y in range(w.nshells):
-            D[o[X]:o[X + 1], o[Y]:o[Y + 1]] *= f[X, Y]
-    return np.ascontiguousarray((D + D.T) / 2)
+_sparse_density = W.sparse_density
 
 
 @pytest.mark.parametrize("cfg", [0, "0b", 1])
