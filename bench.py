@@ -27,11 +27,11 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-PAIR_CLASSES = [(la, lb) for la in range(4) for lb in range(la + 1)]
+PAIR_CLASSES = [(la, lb) for la in range(5) for lb in range(la + 1)]       # up to g: 15 pair classes, 120 quartet classes
 CLASS_NAMES = []
 for X, (la, lb) in enumerate(PAIR_CLASSES):
     for Y, (lc, ld) in enumerate(PAIR_CLASSES[:X + 1]):
-        CLASS_NAMES.append("(%s%s|%s%s)" % ("spdf"[la], "spdf"[lb], "spdf"[lc], "spdf"[ld]))
+        CLASS_NAMES.append("(%s%s|%s%s)" % ("spdfg"[la], "spdfg"[lb], "spdfg"[lc], "spdfg"[ld]))
 
 # classes that run through the block-cooperative Rys kernels (csrc/adft_rys.cu); all others are generated straight-line code
 RYS_CLASSES = {"(fp|fp)", "(ff|pp)", "(fd|dp)", "(ff|fs)", "(fp|dd)", "(fd|fp)", "(ff|dp)", "(fd|dd)", "(ff|fp)", "(fd|fd)",
@@ -237,7 +237,7 @@ def main():
     if rank == 0:
         sampler.start()
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-    step_ms, class_ms, stats = [], np.zeros(55), None
+    step_ms, class_ms, stats = [], np.zeros(len(CLASS_NAMES)), None
     barrier()
     e0.record(stream)
     for _ in range(args.steps):
@@ -312,7 +312,7 @@ def main():
         dom_tflops = cmf[dom] / (class_ms[dom] * 1e-3) / 1e12
         # roofline of the dominant kernel launch: algorithmic (model) FP64 flops of that class launch / its duration
         # measured live with CUDA events on the launching stream (adft_jk_stats.class_ms).  Bound: plain FP64 ALUs.
-        roofline = {"bound": "alu", "kernel": f"{'jk_rys_kernel' if CLASS_NAMES[dom] in RYS_CLASSES else 'jk_kernel'}<{CLASS_NAMES[dom]}>", "kernel_ms": float(class_ms[dom]),
+        roofline = {"bound": "alu", "kernel": f"{'jk_rys_kernel' if (CLASS_NAMES[dom] in RYS_CLASSES or 'g' in CLASS_NAMES[dom]) else 'jk_kernel'}<{CLASS_NAMES[dom]}>", "kernel_ms": float(class_ms[dom]),
                     "kernel_share_of_step": float(class_ms[dom] / ms_step), "kernel_model_flops": float(cmf[dom]),
                     "achieved": dom_tflops, "peak": peak, "unit": "TFLOP/s", "frac": dom_tflops / peak,
                     "whole_step_achieved": step_tflops, "whole_step_frac": step_tflops / peak,
@@ -345,9 +345,9 @@ def main():
                # finalise reads and writes J and K once (4 N^2 doubles); Dmax includes the 16-byte D2H and the host sync
                "phase_gbps": {"finalize": 4.0 * N * N * 8 / (stats.ms_finalize * 1e-3) / 1e9 if stats.ms_finalize > 0 else None,
                               "dmax": N * N * 8 / (stats.ms_dmax * 1e-3) / 1e9 if stats.ms_dmax > 0 else None},
-               "class_ms": {CLASS_NAMES[i]: round(float(class_ms[i]), 3) for i in range(55) if cq[i]},
+               "class_ms": {CLASS_NAMES[i]: round(float(class_ms[i]), 3) for i in range(len(CLASS_NAMES)) if cq[i]},
                "class_model_tflops": {CLASS_NAMES[i]: round(float(cmf[i] / (class_ms[i] * 1e-3) / 1e12), 2)
-                                      for i in range(55) if cq[i] and class_ms[i] > 0},
+                                      for i in range(len(CLASS_NAMES)) if cq[i] and class_ms[i] > 0},
                "roofline": roofline,
                "e2e": {"value": e2e_value, "unit": "quartets/s", "ms_per_step": e2e_ms,
                        "h2d_bytes_per_step": int(N) * N * 8, "d2h_bytes_per_step": 2 * int(N) * N * 8},

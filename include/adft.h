@@ -17,9 +17,9 @@
  * Conventions
  *  - Every function returns adft_status_t (0 = success); nothing throws, aborts or prints.
  *  - "host" pointers are ordinary CPU memory, "device" pointers are CUDA global memory of the current device.
- *  - Units: bohr, Hartree.  Shell angular momentum l = 0..3 (s, p, d, f), Cartesian components.
+ *  - Units: bohr, Hartree.  Shell angular momentum l = 0..4 (s, p, d, f, g), Cartesian components.
  *  - Basis-function order: shells in input order; inside a shell the components (lx,ly,lz) with lx descending,
- *    then ly descending (p: x,y,z; d: xx,xy,xz,yy,yz,zz; f: xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz).
+ *    then ly descending (p: x,y,z; d: xx,xy,xz,yy,yz,zz; f: xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz; g: xxxx,xxxy,...,zzzz).
  *  - All components of a shell share the contraction coefficients d_k:
  *       phi(r) = (x-Ax)^lx (y-Ay)^ly (z-Az)^lz sum_k d_k exp(-alpha_k |r-A|^2).
  *  - There is no CPU fallback: without a CUDA device the compute entry points return ADFT_ERR_CUDA.
@@ -36,7 +36,7 @@ extern "C" {
 typedef enum {
     ADFT_OK = 0,
     ADFT_ERR_INVALID_ARG = 1,   /* NULL pointer, negative size, bad index, non-positive exponent, tau < 0 or NaN */
-    ADFT_ERR_UNSUPPORTED_L = 2, /* a shell has l > 3 (or l < 0) */
+    ADFT_ERR_UNSUPPORTED_L = 2, /* a shell has l > 4 (or l < 0) */
     ADFT_ERR_ALLOC = 3,         /* host or device allocation failed */
     ADFT_ERR_CUDA = 4,          /* CUDA runtime error; text in adft_last_error() */
     ADFT_ERR_NOT_FINITE = 5,    /* D contains NaN or Inf */
@@ -46,7 +46,7 @@ typedef enum {
 /* One shell = one contraction of one angular momentum. */
 typedef struct {
     int32_t atom;         /* index into atom_xyz_bohr */
-    int32_t l;            /* 0..3 */
+    int32_t l;            /* 0..4 */
     int32_t nprim;        /* >= 1 */
     int32_t prim_offset;  /* first primitive of this shell in exponents[] / coefficients[] */
 } adft_shell_t;
@@ -59,7 +59,7 @@ typedef struct adft_shellpairs adft_shellpairs_t; /* opaque; owns every device w
 #define ADFT_NORMALIZE_SHELLS 1u  /* coefficients[] are raw c_k: d_k = c_k N_k / sqrt(S), N_k the primitive norm of
                                      the (L,0,0) component, S its contracted self-overlap (reading R-1) */
 
-#define ADFT_MAX_CLASSES 55       /* quartet classes for l <= 3: 10 pair classes, 10*11/2 */
+#define ADFT_MAX_CLASSES 120      /* quartet classes for l <= 4: 15 pair classes, 15*16/2 (the l <= 3 classes are 0..54) */
 
 /* Counts and device times of the last adft_jk_build on a pairs handle. */
 typedef struct {
@@ -89,7 +89,7 @@ typedef struct {
  *   atom_xyz_bohr [natoms*3], shells [nshells], exponents / coefficients [sum of nprim] (indexed via prim_offset).
  * Errors: NULL / sizes <= 0 / atom index out of range / nprim < 1 or > ADFT_MAX_NPRIM / exponent <= 0 or non-finite
  *         -> INVALID_ARG;
- *         l outside 0..3 -> UNSUPPORTED_L.  *out is written only on success.  Needs no GPU. */
+ *         l outside 0..4 -> UNSUPPORTED_L.  *out is written only on success.  Needs no GPU. */
 adft_status_t adft_basis_create(int32_t natoms, const double *atom_xyz_bohr,
                                 int32_t nshells, const adft_shell_t *shells,
                                 const double *exponents, const double *coefficients,
@@ -193,6 +193,17 @@ adft_status_t adft_jk_build_ex(adft_shellpairs_t *pairs, const double *D, double
  * iterations.  Stats are those of the dD build.  Errors as adft_jk_build; D_prev must not alias D, J or K. */
 adft_status_t adft_jk_build_incremental(adft_shellpairs_t *pairs, const double *D, double *D_prev, double *J, double *K,
                                         double schwarz_threshold, const adft_jk_options_t *options, void *cuda_stream);
+
+/* Spherical-harmonic output.  nsph = sum over shells of 2l+1. */
+adft_status_t adft_basis_nsph(const adft_basis_t *basis, int32_t *nsph);
+
+/* M_sph = T^T M_cart T for a DEVICE N*N matrix in the Cartesian basis (J or K of adft_jk_build): M_sph is a DEVICE
+ * nsph*nsph row-major matrix in the basis of real solid harmonics, shells in input order, m = -l, ..., +l inside a shell
+ * (p: y, z, x;  d: xy, yz, 2zz-xx-yy, xz, xx-yy;  f, g: the textbook forms listed in csrc/adft_sph.cuh), each function
+ * normalised to unit self-overlap given the shell's radial function (the one whose (L,0,0) Cartesian component is
+ * normalised, R-1).  Enqueued on cuda_stream; the first call on a handle synchronises once.
+ * Errors: NULL or aliasing pointers -> INVALID_ARG. */
+adft_status_t adft_cart_to_spherical(adft_shellpairs_t *pairs, const double *M_cart, double *M_sph, void *cuda_stream);
 
 /* Convenience for host callers: D, J, K are HOST N*N arrays; the call stages them through internal device buffers
  * on cuda_stream (host->device copy of D, the build, device->host copies of J and K) and synchronises. */

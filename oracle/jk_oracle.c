@@ -31,13 +31,21 @@
 #include <omp.h>
 #endif
 
+/* Highest shell angular momentum.  liboracle.so is built with 3 (s, p, d, f: the configs of BASELINE.json);
+ * liboracle_g.so is the same source with -DLMAX_SHELL=4 (g shells).  Nothing but the table
+ * sizes below depends on it: the recurrences are written for any L. */
+#ifndef LMAX_SHELL
 #define LMAX_SHELL 3
+#endif
+#define NPC ((LMAX_SHELL + 1) * (LMAX_SHELL + 2) / 2)   /* pair classes (hi >= lo): 10, or 15 with g */
+#define NQC (NPC * (NPC + 1) / 2)                       /* quartet classes: 55, or 120 with g */
 #define MAXM (4 * LMAX_SHELL)                 /* highest Boys order: 12 for (ff|ff) */
 #define NCUM(l) (((l) + 1) * ((l) + 2) * ((l) + 3) / 6)   /* # Cartesian comps of degree <= l; NCUM(-1)=0 */
 #define NCART(l) (((l) + 1) * ((l) + 2) / 2)
-#define NCUM_MAX NCUM(2 * LMAX_SHELL)         /* 84 */
-#define NCUM_B NCUM(LMAX_SHELL)               /* 20 */
-#define NCART_MAX NCART(LMAX_SHELL)           /* 10 */
+#define NCUM_MAX NCUM(2 * LMAX_SHELL)         /* 84 (165 with g) */
+#define NCUM_B NCUM(LMAX_SHELL)               /* 20 (35) */
+#define NCART_MAX NCART(LMAX_SHELL)           /* 10 (15) */
+#define NBLK (NCART_MAX * NCART_MAX * NCART_MAX * NCART_MAX)   /* integrals of one shell quartet */
 
 typedef struct {
     int natoms, nshells;
@@ -185,7 +193,7 @@ int orc_schwarz(BASIS_ARGS, double *Q)
 #pragma omp parallel
     {
         core_scratch_t s;
-        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * 10000);
+        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * NBLK);
         if (core_scratch_alloc(&s) || !blk) {
 #pragma omp atomic write
             err = -3;
@@ -304,15 +312,15 @@ static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, 
     if (pab_hi > npair) pab_hi = npair;
     for (size_t i = 0; i < (size_t)N * N; ++i) Jt[i] = Kt[i] = 0;
     int64_t n_all = 0, n_kept = 0, n_prim = 0;
-    int64_t cc[55]; memset(cc, 0, sizeof cc);
+    int64_t cc[NQC]; memset(cc, 0, sizeof cc);
     int err = 0;
 #pragma omp parallel
     {
         core_scratch_t s;
-        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * 10000);
+        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * NBLK);
         long double *Jp = (long double *)calloc((size_t)N * N, sizeof(long double));
         long double *Kp = (long double *)calloc((size_t)N * N, sizeof(long double));
-        int64_t my_all = 0, my_kept = 0, my_prim = 0, mycc[55];
+        int64_t my_all = 0, my_kept = 0, my_prim = 0, mycc[NQC];
         memset(mycc, 0, sizeof mycc);
         if (core_scratch_alloc(&s) || !blk || !Jp || !Kp) {
 #pragma omp atomic write
@@ -365,7 +373,7 @@ static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, 
             {
                 for (size_t i = 0; i < (size_t)N * N; ++i) { Jt[i] += Jp[i]; Kt[i] += Kp[i]; }
                 n_all += my_all; n_kept += my_kept; n_prim += my_prim;
-                for (int i = 0; i < 55; ++i) cc[i] += mycc[i];
+                for (int i = 0; i < NQC; ++i) cc[i] += mycc[i];
             }
         }
         core_scratch_free(&s); free(blk); free(Jp); free(Kp);
@@ -379,7 +387,7 @@ static int jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, 
 /* ---- exported: screened, 8-fold-symmetric J/K (the oracle proper) ----
  * Q may be NULL (computed here) or a caller-supplied table from orc_schwarz.
  * counts[0] = unique quartets before screening, counts[1] = kept, counts[2] = primitive quartets in kept;
- * class_counts[55] = kept per class.  J, K: full symmetric [nbf*nbf], overwritten. */
+ * class_counts[NQC] = kept per class (55 entries; 120 in the g build).  J, K: full symmetric [nbf*nbf], overwritten. */
 static int jk_full(BASIS_ARGS, const double *D, double tau, const double *Qin, double *J, double *K,
                    int64_t *counts, int64_t *class_counts, int block_density)
 {
@@ -418,9 +426,9 @@ int orc_jk_range(BASIS_ARGS, const double *D, double tau, const double *Qin, int
 static int count_impl(int nshells, const int32_t *l, const int32_t *nprim, const double *Q, double Dmax, const double *Dsh,
                       double tau, int64_t *counts, int64_t *class_counts)
 {
-    int64_t n_all = 0, n_kept = 0, n_prim = 0, cc[55];
+    int64_t n_all = 0, n_kept = 0, n_prim = 0, cc[NQC];
     memset(cc, 0, sizeof cc);
-#pragma omp parallel for schedule(dynamic, 8) reduction(+ : n_all, n_kept, n_prim, cc[:55])
+#pragma omp parallel for schedule(dynamic, 8) reduction(+ : n_all, n_kept, n_prim, cc[:NQC])
     for (int A = 0; A < nshells; ++A)
         for (int B = 0; B <= A; ++B) {
             int64_t pab = (int64_t)A * (A + 1) / 2 + B;
@@ -464,7 +472,7 @@ int orc_jk_brute(BASIS_ARGS, const double *D, double *J, double *K)
     long double *Jt = (long double *)calloc((size_t)N * N, sizeof(long double));
     long double *Kt = (long double *)calloc((size_t)N * N, sizeof(long double));
     core_scratch_t s;
-    CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * 10000);
+    CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * NBLK);
     if (core_scratch_alloc(&s)) return -3;
     for (int A = 0; A < nshells; ++A) for (int B = 0; B < nshells; ++B)
     for (int C = 0; C < nshells; ++C) for (int Dd = 0; Dd < nshells; ++Dd) {
@@ -497,15 +505,15 @@ static int jk_block_impl(BASIS_ARGS, const double *D, double tau, const double *
     bf_offsets(&b, bo);
     const int N = bo[nshells];
     const int nA = NCART(l[sA]), nB = NCART(l[sB]);
-    long double Jt[100], Kt[100];
-    for (int i = 0; i < 100; ++i) Jt[i] = Kt[i] = 0;
+    long double Jt[NCART_MAX * NCART_MAX], Kt[NCART_MAX * NCART_MAX];
+    for (int i = 0; i < NCART_MAX * NCART_MAX; ++i) Jt[i] = Kt[i] = 0;
     int err = 0;
 #pragma omp parallel
     {
         core_scratch_t s;
-        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * 10000);
-        long double Jp[100], Kp[100];
-        for (int i = 0; i < 100; ++i) Jp[i] = Kp[i] = 0;
+        CORE_REAL *blk = (CORE_REAL *)malloc(sizeof(CORE_REAL) * NBLK);
+        long double Jp[NCART_MAX * NCART_MAX], Kp[NCART_MAX * NCART_MAX];
+        for (int i = 0; i < NCART_MAX * NCART_MAX; ++i) Jp[i] = Kp[i] = 0;
         if (core_scratch_alloc(&s) || !blk) {
 #pragma omp atomic write
             err = -3;
@@ -561,6 +569,9 @@ int orc_jk_block_bd(BASIS_ARGS, const double *D, double tau, const double *Q, co
 {
     return jk_block_impl(BASIS_PASS, D, tau, Q, 0.0, Dsh, sA, sB, Jblk, Kblk, work);
 }
+
+int orc_lmax(void) { return LMAX_SHELL; }
+int orc_nqclass(void) { return NQC; }
 
 int orc_num_threads(void)
 {

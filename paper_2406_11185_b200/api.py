@@ -17,7 +17,7 @@ _lib = None
 
 ADFT_COEFFS_FINAL = 0
 ADFT_NORMALIZE_SHELLS = 1
-ADFT_MAX_CLASSES = 55
+ADFT_MAX_CLASSES = 120
 
 STATUS = {0: "ADFT_OK", 1: "ADFT_ERR_INVALID_ARG", 2: "ADFT_ERR_UNSUPPORTED_L", 3: "ADFT_ERR_ALLOC",
           4: "ADFT_ERR_CUDA", 5: "ADFT_ERR_NOT_FINITE", 6: "ADFT_ERR_INTERNAL"}
@@ -52,7 +52,7 @@ class JKOptions(C.Structure):
 ADFT_JK_BLOCK_DENSITY = 1
 ADFT_JK_MIXED_PRECISION = 2
 
-EXPORTS = ["adft_jk_build_ex", "adft_jk_build_incremental", "adft_basis_create", "adft_basis_nbf", "adft_basis_shell_offsets", "adft_basis_coefficients",
+EXPORTS = ["adft_basis_nsph", "adft_cart_to_spherical", "adft_jk_build_ex", "adft_jk_build_incremental", "adft_basis_create", "adft_basis_nbf", "adft_basis_shell_offsets", "adft_basis_coefficients",
            "adft_shellpairs_build", "adft_shellpairs_build_ex", "adft_shellpairs_prim_counts", "adft_shellpairs_schwarz", "adft_jk_build", "adft_jk_build_host", "adft_jk_stats",
            "adft_shellpairs_counts", "adft_shellpairs_destroy", "adft_basis_destroy", "adft_status_string",
            "adft_last_error", "adft_fp64_peak_tflops"]
@@ -73,6 +73,7 @@ def lib():
         L.adft_jk_build_ex.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
         L.adft_jk_build_incremental.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
                                                 C.c_void_p, C.c_void_p]
+        L.adft_cart_to_spherical.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.adft_jk_build_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.adft_shellpairs_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.adft_shellpairs_build_ex.argtypes = [C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
@@ -228,6 +229,18 @@ class ShellPairs:
                                         C.c_void_p(J.ctypes.data) if J is not None else None,
                                         C.c_void_p(K.ctypes.data) if K is not None else None,
                                         C.c_double(tau), _stream_ptr(stream)))
+
+    def cart_to_spherical(self, M, out=None, stream=None):
+        """adft_cart_to_spherical: M [N,N] (J or K) -> [nsph,nsph] in real solid harmonics, m = -l..l inside a shell."""
+        import torch
+        self._check_tensors(M)
+        n = C.c_int32()
+        _check(lib().adft_basis_nsph(self.basis._h, C.byref(n)))
+        if out is None:
+            out = torch.empty(n.value, n.value, dtype=torch.float64, device=M.device)
+        assert out.is_cuda and out.is_contiguous() and tuple(out.shape) == (n.value, n.value) and out.element_size() == 8
+        _check(lib().adft_cart_to_spherical(self._h, C.c_void_p(M.data_ptr()), C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        return out
 
     def stats(self) -> JKStats:
         s = JKStats()

@@ -10,8 +10,9 @@
 
 namespace adft {
 
-constexpr int NPAIRCLASS = 10;     // (la>=lb), la<=3:  pc = la(la+1)/2+lb
-constexpr int NQCLASS = 55;        // X(X+1)/2+Y, X>=Y
+constexpr int NPAIRCLASS = 15;     // (la>=lb), la<=4:  pc = la(la+1)/2+lb
+constexpr int NQCLASS = 120;       // X(X+1)/2+Y, X>=Y
+static_assert(NQCLASS == ADFT_MAX_CLASSES, "adft_jk_stats_t is sized by ADFT_MAX_CLASSES");
 
 inline int pair_class(int la, int lb) { return la * (la + 1) / 2 + lb; }       // requires la >= lb
 inline int quartet_class(int X, int Y) { return X * (X + 1) / 2 + Y; }          // requires X >= Y
@@ -33,6 +34,8 @@ typedef cudaError_t (*rys_sw_fn)(const PairTable &t, const RysTable &rt, int pai
                                  double *Qout, cudaStream_t st);
 rys_jk_fn rys_jk_launcher(int la, int lb, int lc, int ld);
 rys_sw_fn rys_schwarz_launcher(int la, int lb);
+rys_jk_fn rys_jk_launcher_g(int lb, int lc, int ld);      // classes with a g shell on the bra: generated/rys_g_registry.cu
+rys_sw_fn rys_schwarz_launcher_g(int lb);
 ClassEntry *class_table();                    // [NQCLASS]
 void register_all_classes();                  // defined in generated registry.cu
 

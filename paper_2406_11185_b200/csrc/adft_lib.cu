@@ -11,6 +11,7 @@
 
 #include "adft_internal.h"
 #include "adft_rys.cuh"
+#include "adft_sph.cuh"
 
 namespace adft {
 
@@ -290,6 +291,10 @@ struct adft_shellpairs {
     int32_t *d_bfoff = nullptr;               // [nshells+1] first basis function of every shell
     double *d_dsh = nullptr;                  // [nshells*nshells] |D|_XY of the block-density screen (R-23)
     double *d_incr = nullptr;                 // 3 N^2 scratch of adft_jk_build_incremental: dD, J(dD), K(dD)
+    // Cartesian -> spherical output transform (adft_sph.cuh), built on first use
+    SphTables *d_sph = nullptr;
+    int32_t *d_sph_map = nullptr;             // [2*nsph + nshells]: shell of spherical function i, m + l of it, l of every shell
+    int nsph = 0;
 };
 
 // ------------------------------------------------------------------ misc API
@@ -327,8 +332,8 @@ extern "C" adft_status_t adft_basis_create(int32_t natoms, const double *xyz, in
     b->bf_off.push_back(0);
     for (int s = 0; s < nshells; ++s) {
         const adft_shell_t &sh = shells[s];
-        if (sh.l < 0 || sh.l > 3) {
-            set_error("adft_basis_create: shell " + std::to_string(s) + " has l=" + std::to_string(sh.l) + " (supported 0..3)");
+        if (sh.l < 0 || sh.l > 4) {
+            set_error("adft_basis_create: shell " + std::to_string(s) + " has l=" + std::to_string(sh.l) + " (supported 0..4)");
             delete b; return ADFT_ERR_UNSUPPORTED_L;
         }
         if (sh.atom < 0 || sh.atom >= natoms || sh.nprim < 1 || sh.nprim > ADFT_MAX_NPRIM || sh.prim_offset < 0) {
@@ -423,7 +428,7 @@ static void free_pairs(adft_shellpairs *p)
     cudaFree(p->d_off); cudaFree(p->d_Q); cudaFree(p->d_AB); cudaFree(p->d_prim); cudaFree(p->d_pint);
     cudaFree(p->d_boysp); cudaFree(p->d_segs); cudaFree(p->d_counters); cudaFree(p->d_dmax); cudaFree(p->d_stage);
     cudaFree(p->d_rys); cudaFree(p->d_prim_err); cudaFree(p->d_bfoff); cudaFree(p->d_dsh); cudaFree(p->d_incr);
-    cudaFree(p->d_primf); cudaFree(p->d_boysf);
+    cudaFree(p->d_primf); cudaFree(p->d_boysf); cudaFree(p->d_sph); cudaFree(p->d_sph_map);
     if (p->h_segs) cudaFreeHost(p->h_segs);
     if (p->h_small) cudaFreeHost(p->h_small);
     if (p->ev_ok) for (auto &e : p->ev) cudaEventDestroy(e);
@@ -607,11 +612,11 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
         const double *h = adft_rys_blob;
         const int nmax = (int)h[1], ncoef = (int)h[4];
         const int nint = (int)std::lround(h[2] / h[3]);
-        if (h[0] != 5259531.0 || nmax < 7) { set_error("adft_shellpairs_build: bad Rys table blob"); free_pairs(p); return ADFT_ERR_INTERNAL; }
+        if (h[0] != 5259531.0 || nmax != RYS_NMAX) { set_error("adft_shellpairs_build: bad Rys table blob"); free_pairs(p); return ADFT_ERR_INTERNAL; }
         p->rys.tab = p->d_rys; p->rys.nint = nint; p->rys.ncoef = ncoef; p->rys.tmax = h[2]; p->rys.inv_h = 1.0 / h[3];
         int off = 8;
-        for (int n = 1; n <= 7; ++n) { p->rys.off_cheb[n] = off; off += nint * 2 * n * ncoef; }
-        for (int n = 1; n <= 7; ++n) { p->rys.off_asym[n] = off; off += 2 * n; }
+        for (int n = 1; n <= RYS_NMAX; ++n) { p->rys.off_cheb[n] = off; off += nint * 2 * n * ncoef; }
+        for (int n = 1; n <= RYS_NMAX; ++n) { p->rys.off_asym[n] = off; off += 2 * n; }
         if (off != (int)(adft_rys_blob_end - adft_rys_blob)) { set_error("adft_shellpairs_build: Rys table size mismatch"); free_pairs(p); return ADFT_ERR_INTERNAL; }
     }
     if (cudaMallocHost((void **)&p->h_small, 8 * NQCLASS * sizeof(unsigned long long)) != cudaSuccess) {
@@ -1045,6 +1050,45 @@ extern "C" adft_status_t adft_jk_build_host(adft_shellpairs_t *p, const double *
     if (Jh) CUDA_TRY(cudaMemcpyAsync(Jh, dJ, n2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     if (Kh) CUDA_TRY(cudaMemcpyAsync(Kh, dK, n2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_basis_nsph(const adft_basis_t *b, int32_t *nsph)
+{
+    if (!b || !nsph) { set_error("adft_basis_nsph: NULL"); return ADFT_ERR_INVALID_ARG; }
+    int n = 0;
+    for (int l : b->l) n += 2 * l + 1;
+    *nsph = n;
+    return ADFT_OK;
+}
+
+extern "C" adft_status_t adft_cart_to_spherical(adft_shellpairs_t *p, const double *M_cart, double *M_sph, void *cuda_stream)
+{
+    if (!p || !M_cart || !M_sph) { set_error("adft_cart_to_spherical: NULL"); return ADFT_ERR_INVALID_ARG; }
+    if (M_cart == M_sph) { set_error("adft_cart_to_spherical: input and output must not alias"); return ADFT_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const adft_basis *b = p->basis;
+    const int ns = b->nshells;
+    if (!p->d_sph) {
+        std::vector<int32_t> map;
+        for (int s = 0; s < ns; ++s) for (int m = 0; m < 2 * b->l[s] + 1; ++m) map.push_back(s);
+        const int nsph = (int)map.size();
+        for (int s = 0; s < ns; ++s) for (int m = 0; m < 2 * b->l[s] + 1; ++m) map.push_back(m);
+        for (int s = 0; s < ns; ++s) map.push_back(b->l[s]);
+        SphTables tab;
+        sph_fill_tables(tab);
+        CUDA_TRY(cudaMalloc((void **)&p->d_sph, sizeof(SphTables)));
+        CUDA_TRY(cudaMalloc((void **)&p->d_sph_map, map.size() * sizeof(int32_t)));
+        CUDA_TRY(cudaMemcpyAsync(p->d_sph, &tab, sizeof(SphTables), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(p->d_sph_map, map.data(), map.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaStreamSynchronize(st));      // the host copies go out of scope
+        p->nsph = nsph;
+    }
+    const int Ns = p->nsph;
+    dim3 blk(32, 8), grd((Ns + 31) / 32, (Ns + 7) / 8);
+    cart_to_sph_kernel<<<grd, blk, 0, st>>>(M_cart, b->nbf, M_sph, Ns, p->d_sph_map, p->d_sph_map + Ns, p->d_bfoff,
+                                            p->d_sph_map + 2 * Ns, p->d_sph);
+    CUDA_TRY(cudaGetLastError());
     return ADFT_OK;
 }
 

@@ -29,12 +29,13 @@
 
 namespace adft {
 
+constexpr int RYS_NMAX = 9;   // roots of the largest class: (gg|gg), L = 16, L/2 + 1 = 9
 struct RysTable {
     const double *tab;        // device copy of generated/rys_tables.bin (gen_rys.py layout)
     int32_t nint, ncoef;      // intervals on [0, tmax), Chebyshev coefficients per function
     double tmax, inv_h;
-    int32_t off_cheb[8];      // [N]: start of the Chebyshev block of the N-point rule (doubles)
-    int32_t off_asym[8];      // [N]: start of x_i^2 (N values) then h_i (N values)
+    int32_t off_cheb[RYS_NMAX + 1];      // [N]: start of the Chebyshev block of the N-point rule (doubles)
+    int32_t off_asym[RYS_NMAX + 1];      // [N]: start of x_i^2 (N values) then h_i (N values)
 };
 
 // Root r (0-based, ascending) of the NR-point rule: u = t^2 and weight w.
@@ -74,31 +75,31 @@ __host__ __device__ constexpr int rys_cart(int l, int idx, int ax)
         }
     return 0;
 }
-// run-time version through a packed constant (2 bits per exponent, 6 bits per component, l <= 3)
-__host__ __device__ constexpr unsigned long long rys_pack(int l)
-{
-    unsigned long long p = 0ull;
-    for (int idx = 0; idx < rys_ncart(l); ++idx)
-        for (int ax = 0; ax < 3; ++ax) p |= (unsigned long long)rys_cart(l, idx, ax) << (6 * idx + 2 * ax);
-    return p;
-}
+// run-time version: component idx of a shell with angular momentum L sits in row ii = L - lx of the triangle
+// (rows of 1, 2, 3, ... components), ly = ii - (idx - ii(ii+1)/2)
 template <int L>
 __device__ __forceinline__ int rys_cart_rt(int idx, int ax)
 {
-    constexpr unsigned long long P = rys_pack(L);
-    return (int)((P >> (6 * idx + 2 * ax)) & 3ull);
+    int ii = 0;
+#pragma unroll
+    for (int r = 1; r <= L; ++r) ii += (idx >= r * (r + 1) / 2) ? 1 : 0;
+    const int lx = L - ii, ly = ii - (idx - ii * (ii + 1) / 2);
+    return ax == 0 ? lx : (ax == 1 ? ly : L - lx - ly);
 }
 
 // Compile-time description of one class and its thread mapping.
-template <int LA_, int LB_, int LC_, int LD_, int NCH_>
+// NCH thread groups work on NCH chunks of cd component pairs at a time; NPASS > 1 repeats both phases for further chunks
+// (the g classes: (gg|gg) has 225 x 225 integrals per quartet, more than one block can hold in registers at once).
+template <int LA_, int LB_, int LC_, int LD_, int NCH_, int NPASS_ = 1>
 struct RysCfg {
-    static constexpr int LA = LA_, LB = LB_, LC = LC_, LD = LD_, NCH = NCH_;
+    static constexpr int LA = LA_, LB = LB_, LC = LC_, LD = LD_, NCH = NCH_, NPASS = NPASS_;
+    static constexpr int NCHT = NCH * NPASS;                       // cd chunks in total
     static constexpr int NR = (LA + LB + LC + LD) / 2 + 1;
     static constexpr int NA = rys_ncart(LA), NB = rys_ncart(LB), NC = rys_ncart(LC), ND = rys_ncart(LD);
     static constexpr int NAB = NA * NB, NCD = NC * ND;
     static constexpr int NABP = (NAB + 31) / 32 * 32;
     static constexpr int NT = NCH * NABP;                          // threads per block
-    static constexpr int CH = (NCD + NCH - 1) / NCH;               // cd component pairs per thread
+    static constexpr int CH = (NCD + NCHT - 1) / NCHT;             // cd component pairs per thread and pass
     static constexpr int NKL = (LC + 1) * (LD + 1);
     static constexpr int PADCD = NKL | 1;                          // odd stride: the (i,j) slots fall in distinct banks
     // doubles per (item, axis), odd: in phase 1 the 16 lanes of a 64-bit shared-memory wavefront write the same slot of
@@ -266,7 +267,7 @@ __device__ __forceinline__ void rys_phase2_dispatch(int chunk, const double *__r
                                                     int offz, double (&acc)[C::CH])
 {
     if (chunk == CHK) rys_phase2<C, CHK>(sm, nb, offx, offy, offz, acc);
-    else if constexpr (CHK + 1 < C::NCH) rys_phase2_dispatch<C, CHK + 1>(chunk, sm, nb, offx, offy, offz, acc);
+    else if constexpr (CHK + 1 < C::NCHT) rys_phase2_dispatch<C, CHK + 1>(chunk, sm, nb, offx, offy, offz, acc);
 }
 
 // (a5) digestion of the integrals a thread owns: (ia ib | q), q = CHK*CH + n.  Same six updates as DigestJK; WJ / WK
@@ -363,7 +364,7 @@ __device__ __forceinline__ void rys_digest_dispatch(int chunk, const double (&ac
                                                     const JKParams &p, int a0, int b0, int c0, int d0, double wgt, int lane)
 {
     if (chunk == CHK) { RysDigest<C, CHK, WJ, WK> dg; dg.run(acc, active, ia, ib, p, a0, b0, c0, d0, wgt, lane); }
-    else if constexpr (CHK + 1 < C::NCH) rys_digest_dispatch<C, WJ, WK, CHK + 1>(chunk, acc, active, ia, ib, p, a0, b0, c0, d0, wgt, lane);
+    else if constexpr (CHK + 1 < C::NCHT) rys_digest_dispatch<C, WJ, WK, CHK + 1>(chunk, acc, active, ia, ib, p, a0, b0, c0, d0, wgt, lane);
 }
 
 // contracted integrals of one shell quartet into the registers of the block (both phases, all batches)
@@ -399,7 +400,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p
     extern __shared__ double sm[];
     __shared__ long long s_tile;
     const int tid = threadIdx.x, lane = tid & 31;
-    const int chunk = tid / C::NABP, ab = tid - chunk * C::NABP;
+    const int group = tid / C::NABP, ab = tid - group * C::NABP;
     const bool active = ab < C::NAB;
     const int ia = active ? ab / C::NB : 0, ib = active ? ab % C::NB : 0;
     const int offx = (rys_cart_rt<C::LA>(ia, 0) * (C::LB + 1) + rys_cart_rt<C::LB>(ib, 0)) * C::PADCD;
@@ -436,16 +437,19 @@ __global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p
             const int a0 = __ldg(p.t.bfa + gab), b0 = __ldg(p.t.bfb + gab);
             const double AB[3] = {__ldg(p.t.ABx + gab), __ldg(p.t.ABy + gab), __ldg(p.t.ABz + gab)};
             const double CD[3] = {__ldg(p.t.ABx + gcd), __ldg(p.t.ABy + gcd), __ldg(p.t.ABz + gcd)};
-            double acc[C::CH];
-            rys_quartet<C>(p.t, rt, sm, sg.bra_prim_base + i, sg.bra_n, sg.bra_K, sg.ket_prim_base + j, sg.ket_n, sg.ket_K,
-                           AB, CD, chunk, offx, offy, offz, acc);
             const int sa = __ldg(p.t.sha + gab), sb = __ldg(p.t.shb + gab);
             const int sc = __ldg(p.t.sha + gcd), sd = __ldg(p.t.shb + gcd);
             double wgt = 1.0;
             if (sa == sb) wgt *= 0.5;
             if (sc == sd) wgt *= 0.5;
             if (gab == gcd) wgt *= 0.5;
-            rys_digest_dispatch<C, WJ, WK>(chunk, acc, active, ia, ib, p, a0, b0, __ldg(p.t.bfa + gcd), __ldg(p.t.bfb + gcd), wgt, lane);
+            for (int ps = 0; ps < C::NPASS; ++ps) {
+                const int chunk = ps * C::NCH + group;
+                double acc[C::CH];
+                rys_quartet<C>(p.t, rt, sm, sg.bra_prim_base + i, sg.bra_n, sg.bra_K, sg.ket_prim_base + j, sg.ket_n, sg.ket_K,
+                               AB, CD, chunk, offx, offy, offz, acc);
+                rys_digest_dispatch<C, WJ, WK>(chunk, acc, active, ia, ib, p, a0, b0, __ldg(p.t.bfa + gcd), __ldg(p.t.bfb + gcd), wgt, lane);
+            }
         }
     }
     if (tid == 0 && cnt_q) {
@@ -465,7 +469,7 @@ __device__ __forceinline__ double rys_diag_max(int chunk, int ab, const double (
 #pragma unroll
         for (int n = 0; n < C::CH; ++n)
             if (CHK * C::CH + n == ab) m = fabs(acc[n]);
-    } else if constexpr (CHK + 1 < C::NCH) {
+    } else if constexpr (CHK + 1 < C::NCHT) {
         m = rys_diag_max<C, CHK + 1>(chunk, ab, acc);
     }
     return m;
@@ -478,7 +482,7 @@ __global__ void __launch_bounds__(C::NT) schwarz_rys_kernel(const PairTable t, c
     extern __shared__ double sm[];
     __shared__ unsigned long long s_max;
     const int tid = threadIdx.x;
-    const int chunk = tid / C::NABP, ab = tid - chunk * C::NABP;
+    const int group = tid / C::NABP, ab = tid - group * C::NABP;
     const bool active = ab < C::NAB;
     const int ia = active ? ab / C::NB : 0, ib = active ? ab % C::NB : 0;
     const int offx = (rys_cart_rt<C::LA>(ia, 0) * (C::LB + 1) + rys_cart_rt<C::LB>(ib, 0)) * C::PADCD;
@@ -488,10 +492,14 @@ __global__ void __launch_bounds__(C::NT) schwarz_rys_kernel(const PairTable t, c
         const int g = pair_base + j;
         if (tid == 0) s_max = 0ull;
         const double AB[3] = {__ldg(t.ABx + g), __ldg(t.ABy + g), __ldg(t.ABz + g)};
-        double acc[C::CH];
-        rys_quartet<C>(t, rt, sm, prim_base + j, n, K, prim_base + j, n, K, AB, AB, chunk, offx, offy, offz, acc);
-        const double m = active ? rys_diag_max<C>(chunk, ab, acc) : 0.0;
-        if (m > 0.0) atomicMax(&s_max, (unsigned long long)__double_as_longlong(m));
+        __syncthreads();                         // s_max is zero before any thread publishes its maximum
+        for (int ps = 0; ps < C::NPASS; ++ps) {
+            const int chunk = ps * C::NCH + group;
+            double acc[C::CH];
+            rys_quartet<C>(t, rt, sm, prim_base + j, n, K, prim_base + j, n, K, AB, AB, chunk, offx, offy, offz, acc);
+            const double m = active ? rys_diag_max<C>(chunk, ab, acc) : 0.0;
+            if (m > 0.0) atomicMax(&s_max, (unsigned long long)__double_as_longlong(m));
+        }
         __syncthreads();
         if (tid == 0) Qout[g] = sqrt(__longlong_as_double((long long)s_max));
         __syncthreads();

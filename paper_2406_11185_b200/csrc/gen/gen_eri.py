@@ -122,9 +122,23 @@ class VrrDag:
                 t2 = ("T", dec(am, i), c, m, "bra"); self._need(t2)
             self.nodes[key] = ("A", i, d0, d1, am[i], t2)
 
+    def fused_targets(self):
+        """Targets no other node reads: their recurrence is accumulated straight into the contracted sum,
+        acc = fma(PA, d0, acc); acc = fma(WP, d1, acc); ..., one instruction fewer than value + add."""
+        used = set()
+        for s in self.nodes.values():
+            if s[0] == "T":
+                used.update((s[2], s[3]))
+            elif s[0] == "A":
+                used.update(k for k in (s[2], s[3], s[5]) if k)
+            elif s[0] == "K":
+                used.update(k for k in (s[2], s[3], s[5], s[7]) if k)
+        return {("V", a, c, 0) for (a, c) in self.targets
+                if ("V", a, c, 0) not in used and self.nodes[("V", a, c, 0)][0] in ("A", "K")}
+
     # ---- exact FP64-pipe instruction count per primitive quartet (DMUL/DFMA each count 1) ----
     def fp64_ops(self):
-        n = 0
+        n = -len(self.fused_targets())
         for spec in self.nodes.values():
             if spec[0] == "B":
                 n += 1                      # scale F_m by the prefactor
@@ -184,8 +198,21 @@ class VrrDag:
         for n in sorted(used_ze):
             out.append(f"    const R kx{n} = R({float(n)}) * c.inv2ze;")
         tgt_index = {("V", a, cc, 0): j for j, (a, cc) in enumerate(self.targets)}
+        fused = self.fused_targets()
         for key, s in self.nodes.items():
             v = name(key)
+            if key in fused:
+                t = tgt_index[key]
+                if s[0] == "A":
+                    _, i, d0, d1, n2, t2 = s
+                    terms = [(f"c.PA{AX[i]}", name(d0)), (f"c.WP{AX[i]}", name(d1))] + ([(f"kz{n2}", name(t2))] if t2 else [])
+                else:
+                    _, i, d0, d1, n2, t2, nx, tx = s
+                    terms = [(f"c.QC{AX[i]}", name(d0)), (f"c.WQ{AX[i]}", name(d1))] + ([(f"ke{n2}", name(t2))] if t2 else []) \
+                        + ([(f"kx{nx}", name(tx))] if tx else [])
+                for (x, y) in terms:
+                    out.append(f"    acc.template fma<{t}>({x}, {y});")
+                continue
             if s[0] == "B":
                 out.append(f"    const R {v} = F[{s[1]}];")
             elif s[0] == "T":
@@ -406,7 +433,7 @@ def generate_class(la, lb, lc, ld, cmax_list=()):
     return "\n".join(o) + "\n", meta
 
 
-PAIR_CLASSES = [(la, lb) for la in range(4) for lb in range(la + 1)]      # pc = la(la+1)/2+lb, 10 classes
+PAIR_CLASSES = [(la, lb) for la in range(5) for lb in range(la + 1)]      # pc = la(la+1)/2+lb, 15 classes (up to g)
 
 
 def all_classes(lmax=3):
@@ -444,9 +471,11 @@ def main():
     # the library's class table and its model-flop count read this list
     with open(os.path.join(args.out, "class_meta.inc"), "w") as f:
         f.write("// GENERATED: ADFT_CLASS_META(qc, la, lb, lc, ld, vrr_ops, hrr_ops, nint)\n")
-        for (la, lb, lc, ld) in all_classes(3):
+        for (la, lb, lc, ld) in all_classes(4):
             X, Y = la * (la + 1) // 2 + lb, lc * (lc + 1) // 2 + ld
-            v, h = best_vrr(la, lb, lc, ld), HrrDag(la, lb, lc, ld)
+            # (the g classes only need the counts; one direction rule keeps the generation time down)
+            v = best_vrr(la, lb, lc, ld) if la < 4 else VrrDag(la, lb, lc, ld, "first")
+            h = HrrDag(la, lb, lc, ld)
             f.write(f"ADFT_CLASS_META({X * (X + 1) // 2 + Y}, {la}, {lb}, {lc}, {ld}, {v.fp64_ops()}, {h.fp64_ops()}, "
                     f"{ncart(la) * ncart(lb) * ncart(lc) * ncart(ld)})\n")
     # X-macro list of straight-line classes

@@ -24,7 +24,7 @@ import sys
 
 import mpmath as mp
 
-NMAX = 7
+NMAX = 9          # (gg|gg): L = 16, L/2 + 1 = 9 roots
 TMAX = 80.0
 H = 1.0
 NCOEF = 16

@@ -93,13 +93,24 @@ def _draw_shells(rng, atom_kinds, templates, emin, emax, shared=None, nprim_fixe
 
 def _density(rng, nbf, nocc, mode):
     C = rng.standard_normal((nbf, nocc))
-    G = C @ C.T
+    # G = C C^T by rank-1 updates in a fixed order with elementwise IEEE multiplies and adds: bit-identical on every
+    # machine.  (A BLAS matmul picks its kernel, and with it the summation order, by CPU type; stored oracle results are
+    # keyed by the SHA-256 of the inputs and are made on one machine and checked on another.)
+    G = np.zeros((nbf, nbf))
+    tmp = np.empty((nbf, nbf))
+    Ct = np.ascontiguousarray(C.T)
+    for k in range(nocc):
+        np.multiply.outer(Ct[k], Ct[k], out=tmp)
+        G += tmp
     if mode == "cfg0":
         D = 0.2 * G
     elif mode == "over_nocc":
         D = G / float(nocc)
     elif mode == "trace":
-        D = G * (float(nocc) / np.trace(G))
+        tr = 0.0
+        for i in range(nbf):                  # plain sequential sum: np.trace's pairwise blocks are an implementation detail
+            tr += float(G[i, i])
+        D = G * (float(nocc) / tr)
     else:
         raise ValueError(mode)
     return np.ascontiguousarray(0.5 * (D + D.T))
@@ -130,15 +141,26 @@ def _sphere300(rng):
     pts = []
     while len(pts) < n:
         p = rng.uniform(-R, R, size=3)
-        if np.dot(p, p) > R * R:
+        if p[0] * p[0] + p[1] * p[1] + p[2] * p[2] > R * R:
             continue
-        if all(np.dot(p - q, p - q) >= 4.0 for q in pts):
+        if all((p[0] - q[0]) ** 2 + (p[1] - q[1]) ** 2 + (p[2] - q[2]) ** 2 >= 4.0 for q in pts):
             pts.append(p)
     return np.array(pts)
 
 
+_MADE = {}
+
+
 def make(cfg: int | str) -> Workload:
-    """Build config `cfg` in {0, '0b', 1, 2, 3, 4} (BASELINE.json `configs` order; '0b' = R-14 variant)."""
+    """Build config `cfg` in {0, '0b', 1, 2, 3, 4} (BASELINE.json `configs` order; '0b' = R-14 variant).  The result is
+    cached per process (cfg 4 takes 15 s to generate); callers treat it as read-only."""
+    key = str(cfg)
+    if key not in _MADE:
+        _MADE[key] = _make(cfg)
+    return _MADE[key]
+
+
+def _make(cfg: int | str) -> Workload:
     if cfg == "0b":
         idx, variant_b = 0, True
     else:

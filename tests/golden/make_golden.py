@@ -88,7 +88,7 @@ def merge(cfg: int, out: str, parts):
     bs = oracle.basis_from_workload(w)
     N = bs.nbf
     J = np.zeros((N, N), np.longdouble); K = np.zeros((N, N), np.longdouble)
-    cnt = np.zeros(3, np.int64); cc = np.zeros(55, np.int64)
+    cnt = np.zeros(3, np.int64); cc = np.zeros(oracle.NQCLASS, np.int64)
     ranges = []
     nch = None
     for path in parts:
@@ -99,7 +99,7 @@ def merge(cfg: int, out: str, parts):
         ranges.append((int(c["lo"]), int(c["done"])))
         J += c["Jhi"].astype(np.longdouble) + c["Jlo"].astype(np.longdouble)
         K += c["Khi"].astype(np.longdouble) + c["Klo"].astype(np.longdouble)
-        cnt += c["cnt"]; cc += c["cc"]
+        cnt += c["cnt"]; cc[:len(c["cc"])] += c["cc"]        # files written before the g classes existed hold 55 entries
     ranges.sort()
     assert ranges[0][0] == 0 and ranges[-1][1] == nch and all(a[1] == b[0] for a, b in zip(ranges, ranges[1:])), \
         f"partial files do not tile the chunks 0..{nch}: {ranges}"
@@ -117,7 +117,7 @@ def full(cfg: int, out: str, ckpt: str, nchunks: int, max_seconds: float = 0.0, 
     chunks = chunk_bounds(npair, nchunks)
     N = bs.nbf
     J = np.zeros((N, N), np.longdouble); K = np.zeros((N, N), np.longdouble)
-    cnt = np.zeros(3, np.int64); cc = np.zeros(55, np.int64)
+    cnt = np.zeros(3, np.int64); cc = np.zeros(oracle.NQCLASS, np.int64)
     chunk_hi = len(chunks) if chunk_hi < 0 else min(chunk_hi, len(chunks))
     done = chunk_lo
     if ckpt and os.path.exists(ckpt):
@@ -125,7 +125,8 @@ def full(cfg: int, out: str, ckpt: str, nchunks: int, max_seconds: float = 0.0, 
         if str(c["sha"]) == sha and int(c["nchunks"]) == len(chunks) and int(c["lo"]) == chunk_lo:
             J = c["Jhi"].astype(np.longdouble) + c["Jlo"].astype(np.longdouble)
             K = c["Khi"].astype(np.longdouble) + c["Klo"].astype(np.longdouble)
-            cnt, cc, done = c["cnt"], c["cc"], int(c["done"])
+            cnt, done = c["cnt"], int(c["done"])
+            cc[:len(c["cc"])] = c["cc"]
             print(f"resuming after chunk {done}/{len(chunks)}", flush=True)
     for i in range(done, chunk_hi):
         if max_seconds and time.time() - t0 > max_seconds:

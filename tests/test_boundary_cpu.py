@@ -33,7 +33,7 @@ def test_basis_validation_codes(api):
     w = W.make(0)
     sh = w.shells_struct()
     with pytest.raises(api.AdftError) as e:
-        bad = sh.copy(); bad[0, 1] = 4
+        bad = sh.copy(); bad[0, 1] = 5
         api.Basis(w.atoms, bad, w.exponents, w.coefficients)
     assert e.value.status == 2
     with pytest.raises(api.AdftError) as e:

@@ -228,3 +228,32 @@ def test_mixed_precision_errors(api):
             sp.jk_build(D, J, K, 1e-10, mixed_precision=True, fp32_band=band)
         assert e.value.status == 1
     sp.close(); b.close()
+
+
+@pytest.mark.parametrize("cfg", [1, "3cut"])
+def test_spherical_output(api, orc, cfg):
+    """adft_cart_to_spherical: J and K of a build in real solid harmonics against T^T M T of the oracle's
+    J, K with the oracle's independently generated T (oracle/sph.py)."""
+    import torch
+    from oracle import sph
+    if cfg == "3cut":
+        from test_oracle_jk import _first_atoms
+        w = _first_atoms(W.make(3), 8)
+    else:
+        w = W.make(cfg)
+    bs = orc.basis_from_workload(w)
+    Jo, Ko, _ = orc.jk(bs, w.D, w.tau)
+    b = api.Basis.from_workload(w); sp = api.ShellPairs(b)
+    D = torch.from_numpy(w.D).cuda(); J = torch.empty_like(D); K = torch.empty_like(D)
+    sp.jk_build(D, J, K, w.tau)
+    Js = sp.cart_to_spherical(J); Ks = sp.cart_to_spherical(K); torch.cuda.synchronize()
+    nsph = int(sum(2 * int(l) + 1 for l in w.shell_l))
+    assert tuple(Js.shape) == (nsph, nsph)
+    Jso, Kso = sph.cart_to_spherical(w.shell_l, Jo), sph.cart_to_spherical(w.shell_l, Ko)
+    scale = 4 * np.abs(sph.transform_matrix(w.shell_l)).max() ** 2
+    assert np.abs(Js.cpu().numpy() - Jso).max() <= TOL_ELEM * scale and np.abs(Ks.cpu().numpy() - Kso).max() <= TOL_ELEM * scale
+    assert torch.allclose(Js, Js.T, rtol=0, atol=1e-12)
+    with pytest.raises(api.AdftError) as e:
+        api._check(api.lib().adft_cart_to_spherical(sp._h, None, None, None))
+    assert e.value.status == 1
+    sp.close(); b.close()

@@ -101,6 +101,30 @@ def test_class_sweep_f_orderings(api, orc, chunk):
         check_full(api, orc, w, tau=0.0)
 
 
+WIDE_ATOMS = np.array([[0.0, 0.2, -0.3], [3.6, -0.5, 0.8], [-1.9, 6.3, 2.4], [4.4, 5.2, -7.7]])     # 3.7 ... 11.3 bohr apart
+
+
+@pytest.mark.parametrize("chunk", range(9))
+def test_class_sweep_wide_exponents(api, orc, chunk):
+    """The {s,p,d}^4 sweep again in the regime of the configs: exponents log-uniform in [0.05, 5000], atoms 3.7-11.3 bohr
+    apart, tau = 0: tight shells receiving angular momentum from distant diffuse ones (the HRR-cancellation regime behind
+    DESIGN.md R-19 / R-22)."""
+    combos = list(itertools.product(LS, repeat=4))[chunk * 9:(chunk + 1) * 9]
+    for ls in combos:
+        w = W.make_custom(WIDE_ATOMS, [(i, ls[i]) for i in range(4)], seed=7000 + sum(l * 3 ** i for i, l in enumerate(ls)),
+                          emin=0.05, emax=5000.0)
+        check_full(api, orc, w, tau=0.0)
+
+
+@pytest.mark.parametrize("chunk", range(7))
+def test_class_sweep_f_wide_exponents(api, orc, chunk):
+    """The same for all 175 ordered combinations with an f shell."""
+    for ls in F_COMBOS[chunk * 25:(chunk + 1) * 25]:
+        w = W.make_custom(WIDE_ATOMS, [(i, ls[i]) for i in range(4)], seed=9000 + sum(l * 4 ** i for i, l in enumerate(ls)),
+                          emin=0.05, emax=5000.0)
+        check_full(api, orc, w, tau=0.0)
+
+
 @pytest.mark.parametrize("ls", [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (2, 2), (0, 2), (1, 2),
                                 (3, 0), (3, 1), (3, 2), (3, 3), (0, 3), (2, 3)])
 def test_coincident_shells(api, orc, ls):
@@ -236,7 +260,7 @@ def golden_full_parity(api, cfg):
     assert st.dmax == float(g["dmax"])
     assert st.quartets_unique == int(g["unique"])
     assert st.quartets_kept == int(g["kept"]) and st.prim_quartets == int(g["prim"])
-    np.testing.assert_array_equal(np.array(st.class_quartets[:]), g["per_class"])
+    np.testing.assert_array_equal(np.array(st.class_quartets[:]), np.pad(g["per_class"], (0, 120 - len(g["per_class"]))))
     assert np.array_equal(J, J.T) and np.array_equal(K, K.T)
     dj, dk = float(np.abs(J - Jo).max()), float(np.abs(K - Ko).max())
     dEJ, dEK = denergy(w.D, J, Jo, 0.5), denergy(w.D, K, Ko, -0.25)
@@ -268,7 +292,7 @@ def test_cfg4_sampled_parity(api):
     assert st.dmax == float(g["dmax"])
     assert st.quartets_unique == int(g["unique"])
     assert st.quartets_kept == int(g["kept"]) and st.prim_quartets == int(g["prim"])
-    np.testing.assert_array_equal(np.array(st.class_quartets[:]), g["per_class"])
+    np.testing.assert_array_equal(np.array(st.class_quartets[:]), np.pad(g["per_class"], (0, 120 - len(g["per_class"]))))
     o = w.bf_offsets()
     AB = g["AB"]
     assert len(AB) >= 200

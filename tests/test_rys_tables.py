@@ -21,7 +21,7 @@ def tab():
     return gen_rys.read_blob(os.path.join(build.GEN, "rys_tables.bin"))
 
 
-@pytest.mark.parametrize("N", range(1, 8))
+@pytest.mark.parametrize("N", range(1, 10))
 def test_moments_match_oracle_boys(tab, N):
     import gen_rys
     import oracle
@@ -39,4 +39,4 @@ def test_moments_match_oracle_boys(tab, N):
 
 
 def test_table_header(tab):
-    assert tab["nmax"] == 7 and tab["tmax"] == 80.0 and tab["h"] == 1.0 and tab["ncoef"] == 16
+    assert tab["nmax"] == 9 and tab["tmax"] == 80.0 and tab["h"] == 1.0 and tab["ncoef"] == 16
