@@ -768,8 +768,9 @@ static int prefix_len(const double *q, int n, double qfix, double dmax, double t
 // tau_skip > 0 (the fp32 launch of the mixed-precision dispatch, global-Dmax rule only): tile columns that lie, for EVERY
 // row of the segment, inside the fp64 prefix (S >= tau_skip) are left out of the launch.  The last row has the smallest
 // Q_ab and therefore the shortest fp64 prefix; columns below it are fp64 for all rows.
+// tile_c = ket pairs per tile row: TILE_C, or 2*TILE_C for the packed single-precision kernel (two quartets per lane).
 static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax, double tau, std::vector<Segment> &segs,
-                            double tau_skip = 0.0)
+                            double tau_skip = 0.0, int tile_c = TILE_C)
 {
     segs.clear();
     for (int i1 : p->subl_of_class[X])
@@ -786,9 +787,9 @@ static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax,
             Segment sg{};
             sg.bra_pair_base = s1.pair_base; sg.bra_prim_base = s1.prim_base; sg.bra_n = s1.n; sg.bra_K = s1.K;
             sg.ket_pair_base = s2.pair_base; sg.ket_prim_base = s2.prim_base; sg.ket_n = s2.n; sg.ket_K = s2.K;
-            sg.rows = rows; sg.tiles_per_row = (cols + TILE_C - 1) / TILE_C; sg.same = same ? 1 : 0;
+            sg.rows = rows; sg.tiles_per_row = (cols + tile_c - 1) / tile_c; sg.same = same ? 1 : 0;
             if (tau_skip > 0.0) {
-                sg.col_tile_begin = prefix_len(q2, s2.n, q1[rows - 1], dmax, tau_skip) / TILE_C;
+                sg.col_tile_begin = prefix_len(q2, s2.n, q1[rows - 1], dmax, tau_skip) / tile_c;
                 sg.tiles_per_row -= sg.col_tile_begin;
                 if (sg.tiles_per_row <= 0) continue;
             }
@@ -876,7 +877,7 @@ extern "C" adft_status_t adft_jk_build_ex(adft_shellpairs_t *p, const double *D,
             const int qc = quartet_class(X, Y);
             const bool two = mixed && tau > 0.0 && !class_table()[qc].use_rys;
             warps[qc] = plan_class(p, X, Y, dmax, two ? tau64 : tau, plan[qc]);
-            if (two) warps32[qc] = plan_class(p, X, Y, dmax, tau, plan32[qc], block_density ? 0.0 : tau64);
+            if (two) warps32[qc] = plan_class(p, X, Y, dmax, tau, plan32[qc], block_density ? 0.0 : tau64, 2 * TILE_C);
             nseg_total += plan[qc].size() + plan32[qc].size();
         }
     if (nseg_total > p->segs_cap) {
