@@ -32,6 +32,22 @@ __device__ __forceinline__ F2 &operator+=(F2 &a, F2 b) { a.v = __fadd2_rn(a.v, b
 __device__ __forceinline__ F2 fma(F2 a, F2 b, F2 c) { F2 r; r.v = __ffma2_rn(a.v, b.v, c.v); return r; }
 __device__ __forceinline__ F2 fma3(F2 a, F2 b, F2 c) { return fma(a, b, c); }
 
+// primitive-pair record of this kernel: scalars in float, the product centre in double (PairTable::prim, primf4, primf2)
+struct PrimPairF {
+    float zeta, inv2z, PAx, PAy, PAz, cc;
+    double Px, Py, Pz;
+};
+__device__ __forceinline__ PrimPairF load_prim_f(const PairTable &t, int idx)
+{
+    const double *r = reinterpret_cast<const double *>(t.prim + (size_t)(idx >> 3) * 40 + (idx & 7));
+    const float4 a = __ldg(t.primf4 + (size_t)(idx >> 3) * 12 + (idx & 7));
+    const float2 b = __ldg(t.primf2 + (size_t)(idx >> 3) * 24 + 16 + (idx & 7));
+    PrimPairF p;
+    p.zeta = a.x;  p.inv2z = a.y;  p.cc = a.z;  p.PAx = a.w;  p.PAy = b.x;  p.PAz = b.y;
+    p.Px = __ldg(r + 16);  p.Py = __ldg(r + 17);  p.Pz = __ldg(r + 32);          // groups 1 and 2 of the fp64 record
+    return p;
+}
+
 // One primitive quartet for each of the lane's two shell quartets: bra record b, ket records k0 and k1.
 template <class V, class Acc>
 __device__ __forceinline__ void prim_quartet2(const PrimPairF &b, const PrimPairF &k0, const PrimPairF &k1,

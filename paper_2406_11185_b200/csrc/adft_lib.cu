@@ -61,6 +61,7 @@ static void ensure_registered()
     } while (0)
 
 static inline int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+static inline size_t prim_chunks(size_t nprimpairs) { return (nprimpairs + 7) / 8; }      // 8 records per chunk (PairTable::prim)
 #define ADFT_MAX_PRIM_PAIRS (ADFT_MAX_NPRIM * ADFT_MAX_NPRIM)     // primitive pairs of one shell pair the sorter holds
 
 // ------------------------------------------------------------------ small kernels
@@ -117,8 +118,7 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int K, int
                                  const int32_t *__restrict__ shb, const int32_t *__restrict__ sh_atom,
                                  const int32_t *__restrict__ sh_nprim, const int32_t *__restrict__ sh_off,
                                  const double *__restrict__ xyz, const double *__restrict__ expo,
-                                 const double *__restrict__ coef, double *zeta, double *inv2z, double *Px, double *Py,
-                                 double *Pz, double *PAx, double *PAy, double *PAz, double *cc, float *f32, size_t npp)
+                                 const double *__restrict__ coef, double2 *prim, float *primf)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
@@ -149,15 +149,17 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int K, int
         const double iz = 1.0 / z;
         const double px = (a * Ax + b * Bx) * iz, py = (a * Ay + b * By) * iz, pz = (a * Az + b * Bz) * iz;
         const int slot = prim_base + k * n + j;
-        zeta[slot] = z;  inv2z[slot] = 0.5 * iz;
-        Px[slot] = px;  Py[slot] = py;  Pz[slot] = pz;
-        PAx[slot] = px - Ax;  PAy[slot] = py - Ay;  PAz[slot] = pz - Az;
         const double ccv = c0 * ca[ia] * cb[ib] * exp(-a * b * iz * AB2) * iz;
-        cc[slot] = ccv;
-        // single-precision copies for the fp32 launches of the mixed-precision dispatch: zeta, 1/2zeta, P - A, prefactor
-        f32[slot] = (float)z;  f32[npp + slot] = (float)(0.5 * iz);
-        f32[2 * npp + slot] = (float)(px - Ax);  f32[3 * npp + slot] = (float)(py - Ay);  f32[4 * npp + slot] = (float)(pz - Az);
-        f32[5 * npp + slot] = (float)ccv;
+        // chunked record layout of PairTable::prim / primf4 / primf2 (adft_device.cuh)
+        double2 *r = prim + (size_t)(slot >> 3) * 40 + (slot & 7);
+        r[0] = make_double2(z, ccv);
+        r[8] = make_double2(px, py);
+        r[16] = make_double2(pz, 0.5 * iz);
+        r[24] = make_double2(px - Ax, py - Ay);
+        r[32] = make_double2(pz - Az, 0.0);
+        float *f = primf + (size_t)(slot >> 3) * 48;
+        reinterpret_cast<float4 *>(f)[slot & 7] = make_float4((float)z, (float)(0.5 * iz), (float)ccv, (float)(px - Ax));
+        reinterpret_cast<float2 *>(f + 32)[slot & 7] = make_float2((float)(py - Ay), (float)(pz - Az));
     }
 }
 
@@ -265,8 +267,8 @@ struct adft_shellpairs {
     double *d_xyz = nullptr, *d_expo = nullptr, *d_coef = nullptr;
     int32_t *d_atom = nullptr, *d_nprim = nullptr, *d_off = nullptr;
     // device: pair table
-    double *d_Q = nullptr, *d_AB = nullptr /* 3*npairs */, *d_prim = nullptr /* 9*nprimpairs */;
-    float *d_primf = nullptr;                 // 6*nprimpairs single-precision copies (zeta, 1/2zeta, P-A, prefactor)
+    double *d_Q = nullptr, *d_AB = nullptr /* 3*npairs */, *d_prim = nullptr /* chunked records: 80 doubles per 8 slots */;
+    float *d_primf = nullptr;                 // single-precision copies (zeta, 1/2zeta, prefactor, P-A): 48 floats per 8 slots
     float *d_boysf = nullptr;                 // the per-order Boys tables rounded to float (fp32 launches)
     int32_t *d_pint = nullptr /* 5*npairs: bfa,bfb,sha,shb,knom */;
     double *d_boysp = nullptr;                // per-order Taylor tables [BOYS_MORD][BOYS_NT][BOYS_NC] (generated kernels)
@@ -440,17 +442,15 @@ struct HostPair { int sa, sb; double Q; int knom; };
 
 static void set_table_pointers(adft_shellpairs *p)
 {
-    const size_t np = (size_t)p->npairs, npp = (size_t)p->nprimpairs;
+    const size_t np = (size_t)p->npairs;
     PairTable &t = p->tab;
     t.Q = p->d_Q;
     t.ABx = p->d_AB; t.ABy = p->d_AB + np; t.ABz = p->d_AB + 2 * np;
     t.bfa = p->d_pint; t.bfb = p->d_pint + np; t.sha = p->d_pint + 2 * np; t.shb = p->d_pint + 3 * np;
     t.knom = p->d_pint + 4 * np;
-    t.zeta = p->d_prim; t.inv2z = p->d_prim + npp; t.Px = p->d_prim + 2 * npp; t.Py = p->d_prim + 3 * npp;
-    t.Pz = p->d_prim + 4 * npp; t.PAx = p->d_prim + 5 * npp; t.PAy = p->d_prim + 6 * npp; t.PAz = p->d_prim + 7 * npp;
-    t.cc = p->d_prim + 8 * npp;
-    t.zeta_f = p->d_primf; t.inv2z_f = p->d_primf + npp; t.PAx_f = p->d_primf + 2 * npp; t.PAy_f = p->d_primf + 3 * npp;
-    t.PAz_f = p->d_primf + 4 * npp; t.cc_f = p->d_primf + 5 * npp;
+    t.prim = reinterpret_cast<const double2 *>(p->d_prim);
+    t.primf4 = reinterpret_cast<const float4 *>(p->d_primf);
+    t.primf2 = reinterpret_cast<const float2 *>(p->d_primf);
 }
 
 static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vector<HostPair> &hp, double thr, cudaStream_t st)
@@ -469,15 +469,12 @@ static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vecto
     CUDA_TRY(cudaMemcpyAsync(p->d_pint, pint.data(), pint.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemsetAsync(p->d_prim_err, 0, sizeof(int32_t), st));
     CUDA_TRY(cudaStreamSynchronize(st));     // host vectors go out of scope
-    const size_t npp = (size_t)p->nprimpairs;
-    double *f = p->d_prim;
     for (const Sublist &s : p->subl) {
         if (s.n == 0) continue;
         pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.K, s.la, s.lb, thr, nullptr,
                                                              p->d_prim_err, p->tab.sha, p->tab.shb, p->d_atom,
-                                                             p->d_nprim, p->d_off, p->d_xyz, p->d_expo, p->d_coef, f, f + npp,
-                                                             f + 2 * npp, f + 3 * npp, f + 4 * npp, f + 5 * npp, f + 6 * npp,
-                                                             f + 7 * npp, f + 8 * npp, p->d_primf, npp);
+                                                             p->d_nprim, p->d_off, p->d_xyz, p->d_expo, p->d_coef,
+                                                             reinterpret_cast<double2 *>(p->d_prim), p->d_primf);
     }
     CUDA_TRY(cudaGetLastError());
     int32_t bad = 0;
@@ -596,8 +593,8 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     ALLOC(p->d_Q, np * sizeof(double));
     ALLOC(p->d_AB, 3 * np * sizeof(double));
     ALLOC(p->d_pint, 5 * np * sizeof(int32_t));
-    ALLOC(p->d_prim, 9 * npp * sizeof(double));
-    ALLOC(p->d_primf, 6 * npp * sizeof(float));
+    ALLOC(p->d_prim, prim_chunks(npp) * 80 * sizeof(double));
+    ALLOC(p->d_primf, prim_chunks(npp) * 48 * sizeof(float));
     ALLOC(p->d_boysf, (size_t)BOYS_MORD * BOYS_NT * BOYS_NC * sizeof(float));
     ALLOC(p->d_boysp, (size_t)BOYS_MORD * BOYS_NT * BOYS_NC * sizeof(double));
     ALLOC(p->d_counters, 8 * NQCLASS * sizeof(unsigned long long));     // [0,4N) all launches' fp64 part, [4N,8N) fp32 launches
@@ -685,9 +682,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
             if (s.n == 0) continue;
             pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.K, s.la, s.lb, prim_threshold,
                                                                  d_kcount, p->d_prim_err, p->tab.sha, p->tab.shb, p->d_atom, p->d_nprim,
-                                                                 p->d_off, p->d_xyz, p->d_expo, p->d_coef, nullptr, nullptr,
-                                                                 nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
-                                                                 nullptr, 0);
+                                                                 p->d_off, p->d_xyz, p->d_expo, p->d_coef, nullptr, nullptr);
         }
         TRY2(cudaGetLastError());
         std::vector<int32_t> kc(np);
@@ -703,10 +698,10 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
         if (p->nprimpairs < p->nprimpairs_nominal) {      // compact table: release the records of the dropped primitives
             TRY2(cudaFree(p->d_prim));
             p->d_prim = nullptr;
-            TRY2(cudaMalloc((void **)&p->d_prim, 9 * (size_t)p->nprimpairs * sizeof(double)));
+            TRY2(cudaMalloc((void **)&p->d_prim, prim_chunks((size_t)p->nprimpairs) * 80 * sizeof(double)));
             TRY2(cudaFree(p->d_primf));
             p->d_primf = nullptr;
-            TRY2(cudaMalloc((void **)&p->d_primf, 6 * (size_t)p->nprimpairs * sizeof(float)));
+            TRY2(cudaMalloc((void **)&p->d_primf, prim_chunks((size_t)p->nprimpairs) * 48 * sizeof(float)));
         }
         set_table_pointers(p);
     }

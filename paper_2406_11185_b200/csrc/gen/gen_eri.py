@@ -136,9 +136,14 @@ class VrrDag:
         return {("V", a, c, 0) for (a, c) in self.targets
                 if ("V", a, c, 0) not in used and self.nodes[("V", a, c, 0)][0] in ("A", "K")}
 
-    # ---- exact FP64-pipe instruction count per primitive quartet (DMUL/DFMA each count 1) ----
+    # ---- FP64 operation count per primitive quartet of the recurrence in its canonical form (every node a value, one
+    # add per contracted target; DMUL/DFMA/DADD each count 1): the MODEL count of DESIGN.md R-21, unchanged since round 1.
+    # The emitted code executes len(fused_targets()) instructions fewer (fp64_instr).
+    def fp64_instr(self):
+        return self.fp64_ops() - len(self.fused_targets())
+
     def fp64_ops(self):
-        n = -len(self.fused_targets())
+        n = 0
         for spec in self.nodes.values():
             if spec[0] == "B":
                 n += 1                      # scale F_m by the prefactor
@@ -342,7 +347,7 @@ def best_vrr(la, lb, lc, ld, targets=None):
     best = None
     for how in ("first", "last", "max", "min"):
         d = VrrDag(la, lb, lc, ld, how, targets)
-        if best is None or d.fp64_ops() < best.fp64_ops():
+        if best is None or d.fp64_instr() < best.fp64_instr():
             best = d
     return best
 
@@ -365,7 +370,7 @@ def plan_passes(la, lb, lc, ld, cmax):
             for i in range(0, len(clist), g):
                 tg = [(a, c) for a in alist for c in clist[i:i + g]]
                 passes.append(best_vrr(la, lb, lc, ld, tg))
-        cost = sum(p.fp64_ops() + PREAMBLE_OPS for p in passes)
+        cost = sum(p.fp64_instr() + PREAMBLE_OPS for p in passes)
         if best is None or cost < best_cost:
             best, best_cost = passes, cost
     return best
@@ -380,7 +385,8 @@ def generate_class(la, lb, lc, ld, cmax_list=()):
     nint = ncart(la) * ncart(lb) * ncart(lc) * ncart(ld)
     o = []
     o.append(f"// GENERATED by csrc/gen/gen_eri.py -- class ({'spdf'[la]}{'spdf'[lb]}|{'spdf'[lc]}{'spdf'[ld]}); do not edit.")
-    o.append(f"// VRR: {len(vrr.nodes)} nodes, {vrr.fp64_ops()} FP64 ops per primitive quartet (direction rule '{vrr.how}');")
+    o.append(f"// VRR: {len(vrr.nodes)} nodes, {vrr.fp64_ops()} FP64 operations per primitive quartet in canonical form (the model count), "
+             f"{vrr.fp64_instr()} instructions emitted (direction rule '{vrr.how}');")
     o.append(f"// HRR: {hrr.fp64_ops()} FP64 ops per contracted quartet; {nint} integrals.")
     o.append("#pragma once")
     o.append(f"struct G_{tag} {{")

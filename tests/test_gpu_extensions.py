@@ -258,3 +258,30 @@ def test_spherical_output(api, orc, cfg):
         api._check(api.lib().adft_cart_to_spherical(sp._h, None, None, None))
     assert e.value.status == 1
     sp.close(); b.close()
+
+
+def test_options_combined(api, orc):
+    """Mixed precision together with the block-density screen and with sharding: the kept set is still the oracle's (block
+    rule), every quartet is evaluated exactly once across precisions and ranks."""
+    import torch
+    w = W.make(1)
+    D = W.sparse_density(w, 21, decades=4.0)
+    bs = orc.basis_from_workload(w)
+    Qo = orc.schwarz(bs)
+    tau = 1e-10
+    Jo, Ko, cnt = orc.jk(bs, D, tau, Qo, block_density=True)
+    b = api.Basis.from_workload(w); sp = api.ShellPairs(b)
+    tD = torch.from_numpy(D).cuda()
+    Js = torch.zeros_like(tD); Ks = torch.zeros_like(tD)
+    counts = np.zeros(120, np.int64); n32 = 0
+    for r in range(2):
+        J = torch.empty_like(tD); K = torch.empty_like(tD)
+        sp.jk_build(tD, J, K, tau, block_density=True, mixed_precision=True, shard=(r, 2)); torch.cuda.synchronize()
+        st = sp.stats()
+        counts += np.array(st.class_quartets[:]); n32 += st.quartets_fp32
+        Js += J; Ks += K
+    np.testing.assert_array_equal(counts, cnt["per_class"])
+    assert 0 < n32 < cnt["kept"]
+    tol = mixed_tolerance(bs.nshells * (bs.nshells + 1) // 2, tau, 1e5)
+    assert np.abs(Js.cpu().numpy() - Jo).max() <= tol and np.abs(Ks.cpu().numpy() - Ko).max() <= tol
+    sp.close(); b.close()
