@@ -9,7 +9,8 @@
  *
  * evaluated on the fly over the unique shell quartets (8-fold permutational symmetry) that pass
  *     (Q_AB * Q_CD) * max|D|  >=  schwarz_threshold ,   Q_AB = sqrt(max_{mu in A, nu in B} |(mu nu|mu nu)|)
- * ("If S(AB|CD) < TOLERANCE -> there will not be dispatch").  All arithmetic is fp64.
+ * ("If S(AB|CD) < TOLERANCE -> there will not be dispatch").  All arithmetic is fp64 unless the caller asks
+ * for the paper's mixed-precision dispatch (ADFT_JK_MIXED_PRECISION of adft_jk_build_ex).
  *
  * Call sequence:  adft_basis_create -> adft_shellpairs_build -> adft_jk_build (any number of times)
  *                 -> adft_shellpairs_destroy -> adft_basis_destroy.

@@ -32,7 +32,7 @@ __device__ __forceinline__ F2 &operator+=(F2 &a, F2 b) { a.v = __fadd2_rn(a.v, b
 __device__ __forceinline__ F2 fma(F2 a, F2 b, F2 c) { F2 r; r.v = __ffma2_rn(a.v, b.v, c.v); return r; }
 __device__ __forceinline__ F2 fma3(F2 a, F2 b, F2 c) { return fma(a, b, c); }
 
-// primitive-pair record of this kernel: scalars in float, the product centre in double (PairTable::prim, primf4, primf2)
+// primitive-pair record of this kernel: scalars in float, the product centre in double (PairTable::prim, primf)
 struct PrimPairF {
     float zeta, inv2z, PAx, PAy, PAz, cc;
     double Px, Py, Pz;
@@ -40,10 +40,12 @@ struct PrimPairF {
 __device__ __forceinline__ PrimPairF load_prim_f(const PairTable &t, int idx)
 {
     const double *r = reinterpret_cast<const double *>(t.prim + (size_t)(idx >> 3) * 40 + (idx & 7));
-    const float4 a = __ldg(t.primf4 + (size_t)(idx >> 3) * 12 + (idx & 7));
-    const float2 b = __ldg(t.primf2 + (size_t)(idx >> 3) * 24 + 16 + (idx & 7));
+    const float *f = t.primf + idx;
+    const size_t n = t.primf_stride;
     PrimPairF p;
-    p.zeta = a.x;  p.inv2z = a.y;  p.cc = a.z;  p.PAx = a.w;  p.PAy = b.x;  p.PAz = b.y;
+    p.zeta = __ldg(f);  p.inv2z = __ldg(f + n);
+    p.PAx = __ldg(f + 2 * n);  p.PAy = __ldg(f + 3 * n);  p.PAz = __ldg(f + 4 * n);
+    p.cc = __ldg(f + 5 * n);
     p.Px = __ldg(r + 16);  p.Py = __ldg(r + 17);  p.Pz = __ldg(r + 32);          // groups 1 and 2 of the fp64 record
     return p;
 }

@@ -118,7 +118,7 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int K, int
                                  const int32_t *__restrict__ shb, const int32_t *__restrict__ sh_atom,
                                  const int32_t *__restrict__ sh_nprim, const int32_t *__restrict__ sh_off,
                                  const double *__restrict__ xyz, const double *__restrict__ expo,
-                                 const double *__restrict__ coef, double2 *prim, float *primf)
+                                 const double *__restrict__ coef, double2 *prim, float *primf, size_t npp)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
@@ -150,16 +150,16 @@ __global__ void pair_prim_kernel(int pair_base, int prim_base, int n, int K, int
         const double px = (a * Ax + b * Bx) * iz, py = (a * Ay + b * By) * iz, pz = (a * Az + b * Bz) * iz;
         const int slot = prim_base + k * n + j;
         const double ccv = c0 * ca[ia] * cb[ib] * exp(-a * b * iz * AB2) * iz;
-        // chunked record layout of PairTable::prim / primf4 / primf2 (adft_device.cuh)
+        // chunked record layout of PairTable::prim, one float array per field in primf (adft_device.cuh)
         double2 *r = prim + (size_t)(slot >> 3) * 40 + (slot & 7);
         r[0] = make_double2(z, ccv);
         r[8] = make_double2(px, py);
         r[16] = make_double2(pz, 0.5 * iz);
         r[24] = make_double2(px - Ax, py - Ay);
         r[32] = make_double2(pz - Az, 0.0);
-        float *f = primf + (size_t)(slot >> 3) * 48;
-        reinterpret_cast<float4 *>(f)[slot & 7] = make_float4((float)z, (float)(0.5 * iz), (float)ccv, (float)(px - Ax));
-        reinterpret_cast<float2 *>(f + 32)[slot & 7] = make_float2((float)(py - Ay), (float)(pz - Az));
+        primf[slot] = (float)z;  primf[npp + slot] = (float)(0.5 * iz);
+        primf[2 * npp + slot] = (float)(px - Ax);  primf[3 * npp + slot] = (float)(py - Ay);  primf[4 * npp + slot] = (float)(pz - Az);
+        primf[5 * npp + slot] = (float)ccv;
     }
 }
 
@@ -268,7 +268,7 @@ struct adft_shellpairs {
     int32_t *d_atom = nullptr, *d_nprim = nullptr, *d_off = nullptr;
     // device: pair table
     double *d_Q = nullptr, *d_AB = nullptr /* 3*npairs */, *d_prim = nullptr /* chunked records: 80 doubles per 8 slots */;
-    float *d_primf = nullptr;                 // single-precision copies (zeta, 1/2zeta, prefactor, P-A): 48 floats per 8 slots
+    float *d_primf = nullptr;                 // single-precision copies, one array per field: 6*nprimpairs floats
     float *d_boysf = nullptr;                 // the per-order Boys tables rounded to float (fp32 launches)
     int32_t *d_pint = nullptr /* 5*npairs: bfa,bfb,sha,shb,knom */;
     double *d_boysp = nullptr;                // per-order Taylor tables [BOYS_MORD][BOYS_NT][BOYS_NC] (generated kernels)
@@ -449,8 +449,8 @@ static void set_table_pointers(adft_shellpairs *p)
     t.bfa = p->d_pint; t.bfb = p->d_pint + np; t.sha = p->d_pint + 2 * np; t.shb = p->d_pint + 3 * np;
     t.knom = p->d_pint + 4 * np;
     t.prim = reinterpret_cast<const double2 *>(p->d_prim);
-    t.primf4 = reinterpret_cast<const float4 *>(p->d_primf);
-    t.primf2 = reinterpret_cast<const float2 *>(p->d_primf);
+    t.primf = p->d_primf;
+    t.primf_stride = (size_t)p->nprimpairs;
 }
 
 static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vector<HostPair> &hp, double thr, cudaStream_t st)
@@ -474,7 +474,7 @@ static adft_status_t upload_pairs_and_prims(adft_shellpairs *p, const std::vecto
         pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.K, s.la, s.lb, thr, nullptr,
                                                              p->d_prim_err, p->tab.sha, p->tab.shb, p->d_atom,
                                                              p->d_nprim, p->d_off, p->d_xyz, p->d_expo, p->d_coef,
-                                                             reinterpret_cast<double2 *>(p->d_prim), p->d_primf);
+                                                             reinterpret_cast<double2 *>(p->d_prim), p->d_primf, (size_t)p->nprimpairs);
     }
     CUDA_TRY(cudaGetLastError());
     int32_t bad = 0;
@@ -594,7 +594,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
     ALLOC(p->d_AB, 3 * np * sizeof(double));
     ALLOC(p->d_pint, 5 * np * sizeof(int32_t));
     ALLOC(p->d_prim, prim_chunks(npp) * 80 * sizeof(double));
-    ALLOC(p->d_primf, prim_chunks(npp) * 48 * sizeof(float));
+    ALLOC(p->d_primf, 6 * npp * sizeof(float));
     ALLOC(p->d_boysf, (size_t)BOYS_MORD * BOYS_NT * BOYS_NC * sizeof(float));
     ALLOC(p->d_boysp, (size_t)BOYS_MORD * BOYS_NT * BOYS_NC * sizeof(double));
     ALLOC(p->d_counters, 8 * NQCLASS * sizeof(unsigned long long));     // [0,4N) all launches' fp64 part, [4N,8N) fp32 launches
@@ -682,7 +682,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
             if (s.n == 0) continue;
             pair_prim_kernel<<<(s.n + 127) / 128, 128, 0, st>>>(s.pair_base, s.prim_base, s.n, s.K, s.la, s.lb, prim_threshold,
                                                                  d_kcount, p->d_prim_err, p->tab.sha, p->tab.shb, p->d_atom, p->d_nprim,
-                                                                 p->d_off, p->d_xyz, p->d_expo, p->d_coef, nullptr, nullptr);
+                                                                 p->d_off, p->d_xyz, p->d_expo, p->d_coef, nullptr, nullptr, 0);
         }
         TRY2(cudaGetLastError());
         std::vector<int32_t> kc(np);
@@ -701,7 +701,7 @@ extern "C" adft_status_t adft_shellpairs_build_ex(const adft_basis_t *b, double 
             TRY2(cudaMalloc((void **)&p->d_prim, prim_chunks((size_t)p->nprimpairs) * 80 * sizeof(double)));
             TRY2(cudaFree(p->d_primf));
             p->d_primf = nullptr;
-            TRY2(cudaMalloc((void **)&p->d_primf, prim_chunks((size_t)p->nprimpairs) * 48 * sizeof(float)));
+            TRY2(cudaMalloc((void **)&p->d_primf, 6 * (size_t)p->nprimpairs * sizeof(float)));
         }
         set_table_pointers(p);
     }

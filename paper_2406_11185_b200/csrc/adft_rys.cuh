@@ -57,7 +57,7 @@ __device__ __forceinline__ void rys_root(const RysTable &rt, double T, int r, do
         u = fma(x, b1, __ldg(cu) - b2);
         w = fma(x, d1, __ldg(cw) - d2);
     } else {
-        const double ri = rsqrt(T);
+        const double ri = rsqrt_normal(T);
         u = __ldg(rt.tab + rt.off_asym[NR] + r) * ri * ri;
         w = __ldg(rt.tab + rt.off_asym[NR] + NR + r) * ri;
     }
@@ -128,7 +128,7 @@ __device__ __forceinline__ void rys_phase1(const RysTable &rt, const PrimPair &b
 {
     constexpr int NBR = C::LA + C::LB, NKT = C::LC + C::LD;
     const double s = b.zeta + k.zeta;
-    const double rs = rsqrt(s);
+    const double rs = rsqrt_normal(s);
     const double inv_s = rs * rs;
     const double roz = k.zeta * inv_s, roe = b.zeta * inv_s;      // rho/zeta, rho/eta
     const double rho = b.zeta * roz;

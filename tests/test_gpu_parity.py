@@ -280,13 +280,11 @@ def test_cfg3_full_parity(api):
     golden_full_parity(api, 3)
 
 
-def test_cfg4_sampled_parity(api):
-    """cfg 4 (300 atoms, 2500 functions, tau = 1e-11): the workload and launch configuration bench.py times.  Equal
-    per-class kept counts (6.17e9 quartets) and 207 stored J/K shell blocks, 23 of every ordered block type
-    (l_A, l_B) in {s,p,d}^2, each evaluated by the oracle from the definition with the same screen.  Sampled:
-    element parity on the samples, energy parity NOT claimed for this config (the full oracle is a day of CPU time)."""
-    w = W.make(4)
-    g = load_golden("cfg4_blocks.npz", w)
+def golden_sampled_parity(api, cfg, fname, ntypes, per_type_min, nmin):
+    """Equal per-class kept counts and stored J/K shell blocks, stratified over the ordered block types (l_A, l_B), each
+    evaluated by the oracle from the definition with the same screen (oracle.jk_block)."""
+    w = W.make(cfg)
+    g = load_golden(fname, w)
     J, K, st, Q = api.jk(w)
     check_q(Q, g["Q"])
     assert st.dmax == float(g["dmax"])
@@ -295,7 +293,7 @@ def test_cfg4_sampled_parity(api):
     np.testing.assert_array_equal(np.array(st.class_quartets[:]), np.pad(g["per_class"], (0, 120 - len(g["per_class"]))))
     o = w.bf_offsets()
     AB = g["AB"]
-    assert len(AB) >= 200
+    assert len(AB) >= nmin
     types = {}
     worst = 0.0
     for (A, B), Jb, Kb in zip(AB, g["J_blocks"], g["K_blocks"]):
@@ -303,11 +301,25 @@ def test_cfg4_sampled_parity(api):
         types[(int(w.shell_l[A]), int(w.shell_l[B]))] = types.get((int(w.shell_l[A]), int(w.shell_l[B])), 0) + 1
         worst = max(worst, np.abs(J[o[A]:o[A + 1], o[B]:o[B + 1]] - Jb[:na, :nb]).max(),
                     np.abs(K[o[A]:o[A + 1], o[B]:o[B + 1]] - Kb[:na, :nb]).max())
-    assert len(types) == 9 and min(types.values()) >= 20
-    print(f"cfg 4 sampled parity: {len(AB)} blocks, worst |dJ|,|dK| {worst:.2e}")
+    assert len(types) == ntypes and min(types.values()) >= per_type_min
+    print(f"cfg {cfg} sampled parity: {len(AB)} blocks, worst |dJ|,|dK| {worst:.2e}")
     assert worst <= TOL_ELEM, worst
     assert np.array_equal(J, J.T) and np.array_equal(K, K.T)
     assert np.sum(w.D * J) > 0 and np.sum(w.D * K) > 0
+
+
+def test_cfg4_sampled_parity(api):
+    """cfg 4 (300 atoms, 2500 functions, tau = 1e-11): the workload and launch configuration bench.py times.  Equal
+    per-class kept counts (6.17e9 quartets) and 207 stored J/K shell blocks, 23 of every ordered block type
+    (l_A, l_B) in {s,p,d}^2.  Sampled: element parity on the samples, energy parity NOT claimed for this config (the full
+    oracle is a day of CPU time)."""
+    golden_sampled_parity(api, 4, "cfg4_blocks.npz", 9, 20, 200)
+
+
+def test_cfg3_sampled_parity(api):
+    """cfg 3 (f shells, 940 functions, all 55 classes of l <= 3, 4.8e8 kept quartets): per-class kept counts and 208 stored
+    J/K shell blocks, 13 of every ordered block type in {s,p,d,f}^2."""
+    golden_sampled_parity(api, 3, "cfg3_blocks.npz", 16, 12, 200)
 
 
 def test_degenerate_inputs(api, orc):
