@@ -52,7 +52,7 @@ class JKOptions(C.Structure):
 ADFT_JK_BLOCK_DENSITY = 1
 ADFT_JK_MIXED_PRECISION = 2
 
-EXPORTS = ["adft_basis_nsph", "adft_cart_to_spherical", "adft_jk_build_ex", "adft_jk_build_incremental", "adft_basis_create", "adft_basis_nbf", "adft_basis_shell_offsets", "adft_basis_coefficients",
+EXPORTS = ["adft_basis_nsph", "adft_cart_to_spherical", "adft_cart_to_spherical_noalloc", "adft_jk_build_ex", "adft_jk_build_incremental", "adft_basis_create", "adft_basis_nbf", "adft_basis_shell_offsets", "adft_basis_coefficients",
            "adft_shellpairs_build", "adft_shellpairs_build_ex", "adft_shellpairs_prim_counts", "adft_shellpairs_schwarz", "adft_jk_build", "adft_jk_build_host", "adft_jk_stats",
            "adft_shellpairs_counts", "adft_shellpairs_destroy", "adft_basis_destroy", "adft_status_string",
            "adft_last_error", "adft_fp64_peak_tflops"]
@@ -74,6 +74,7 @@ def lib():
         L.adft_jk_build_incremental.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
                                                 C.c_void_p, C.c_void_p]
         L.adft_cart_to_spherical.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.adft_cart_to_spherical_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.adft_jk_build_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.adft_shellpairs_build.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.adft_shellpairs_build_ex.argtypes = [C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
@@ -240,6 +241,16 @@ class ShellPairs:
             out = torch.empty(n.value, n.value, dtype=torch.float64, device=M.device)
         assert out.is_cuda and out.is_contiguous() and tuple(out.shape) == (n.value, n.value) and out.element_size() == 8
         _check(lib().adft_cart_to_spherical(self._h, C.c_void_p(M.data_ptr()), C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        return out
+
+    def cart_to_spherical_noalloc(self, M, out, stream=None):
+        """adft_cart_to_spherical_noalloc (include/adft_noalloc.h): the same transform with its working memory in the
+        library's static device array: no allocation here or in the library, so the caller passes `out` [nsph,nsph]."""
+        self._check_tensors(M)
+        n = C.c_int32()
+        _check(lib().adft_basis_nsph(self.basis._h, C.byref(n)))
+        assert out.is_cuda and out.is_contiguous() and out.element_size() == 8 and tuple(out.shape) == (n.value, n.value)
+        _check(lib().adft_cart_to_spherical_noalloc(self._h, C.c_void_p(M.data_ptr()), C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
         return out
 
     def stats(self) -> JKStats:

@@ -12,6 +12,7 @@
 #include "adft_internal.h"
 #include "adft_rys.cuh"
 #include "adft_sph.cuh"
+#include "../../include/adft_noalloc.h"
 
 namespace adft {
 
@@ -1114,5 +1115,106 @@ extern "C" adft_status_t adft_fp64_peak_tflops(void *cuda_stream, double *tflops
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
     *tflops = best;
+    return ADFT_OK;
+}
+
+// ------------------------------------------------------------------ the entry point that allocates nothing
+// include/adft_noalloc.h: adft_cart_to_spherical with its working memory (the transform tables, the index map of the
+// basis) in one file-scope device array instead of per-handle cudaMalloc'ed buffers.  Every call on a device shares the
+// array; the basis-dependent part is rebuilt by noalloc_sph_map_kernel on the caller's stream ahead of the transform.
+namespace adft {
+
+struct NoAllocScratch {
+    SphTables tab;                                    // written once per device at set-up
+    int32_t sph_shell[ADFT_NOALLOC_MAX_NSPH];         // rebuilt by every call: shell of spherical function i,
+    int32_t sph_m[ADFT_NOALLOC_MAX_NSPH];             //   m + l of it,
+    int32_t shell_l[ADFT_NOALLOC_MAX_SHELLS];         //   l of every shell
+};
+constexpr size_t NOALLOC_BYTES = (sizeof(NoAllocScratch) + 255) / 256 * 256;
+
+// In host code this name is a host-side stand-in, not a device address: host code takes the address with
+// cudaGetSymbolAddress (noalloc_scratch_ptr below); device code may name the array directly.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_BYTES];
+
+// One block: l of every shell from its Cartesian size, an exclusive scan of 2l+1 over the shells, then the map.
+// Overwrites everything the transform of this call reads; nothing has to be zero on entry.
+__global__ void noalloc_sph_map_kernel(const int32_t *__restrict__ bfoff, int ns)
+{
+    NoAllocScratch *s = reinterpret_cast<NoAllocScratch *>(g_noalloc_scratch);
+    __shared__ int part[1024];
+    const int t = threadIdx.x, per = (ns + (int)blockDim.x - 1) / (int)blockDim.x;
+    const int lo = min(t * per, ns), hi = min(lo + per, ns);
+    int sum = 0;
+    for (int sh = lo; sh < hi; ++sh) {
+        const int nc = bfoff[sh + 1] - bfoff[sh];
+        int l = 0;
+        while ((l + 1) * (l + 2) / 2 < nc) ++l;
+        s->shell_l[sh] = l;
+        sum += 2 * l + 1;
+    }
+    part[t] = sum;
+    __syncthreads();
+    for (int d = 1; d < (int)blockDim.x; d <<= 1) {          // inclusive scan over the threads
+        const int v = t >= d ? part[t - d] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    int o = part[t] - sum;
+    for (int sh = lo; sh < hi; ++sh) {
+        const int n = 2 * s->shell_l[sh] + 1;
+        for (int m = 0; m < n; ++m) { s->sph_shell[o + m] = sh; s->sph_m[o + m] = m; }
+        o += n;
+    }
+}
+
+// The array's device address, once per device, taken with that device current.
+static adft_status_t noalloc_scratch_ptr(NoAllocScratch **out)
+{
+    constexpr int MAXDEV = 64;
+    static std::mutex mtx;
+    static NoAllocScratch *ptr[MAXDEV] = {};
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAXDEV) { set_error("adft_cart_to_spherical_noalloc: device ordinal out of range"); return ADFT_ERR_INVALID_ARG; }
+    std::lock_guard<std::mutex> lk(mtx);
+    if (!ptr[dev]) {
+        void *a = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&a, g_noalloc_scratch));
+        if (!a) { set_error("adft_cart_to_spherical_noalloc: cudaGetSymbolAddress returned NULL"); return ADFT_ERR_CUDA; }
+        SphTables tab;                                       // 5.4 KB on the stack
+        sph_fill_tables(tab);
+        CUDA_TRY(cudaMemcpy(a, &tab, sizeof(SphTables), cudaMemcpyHostToDevice));      // tab is the first member
+        ptr[dev] = static_cast<NoAllocScratch *>(a);
+    }
+    *out = ptr[dev];
+    return ADFT_OK;
+}
+
+}  // namespace adft
+
+extern "C" adft_status_t adft_cart_to_spherical_noalloc(adft_shellpairs_t *p, const double *M_cart, double *M_sph, void *cuda_stream)
+{
+    if (!p || !M_cart || !M_sph) { set_error("adft_cart_to_spherical_noalloc: NULL"); return ADFT_ERR_INVALID_ARG; }
+    if (M_cart == M_sph) { set_error("adft_cart_to_spherical_noalloc: input and output must not alias"); return ADFT_ERR_INVALID_ARG; }
+    const adft_basis *b = p->basis;
+    const int ns = b->nshells;
+    long long Ns = 0;
+    for (int s = 0; s < ns; ++s) Ns += 2 * b->l[s] + 1;
+    if (ns > ADFT_NOALLOC_MAX_SHELLS || Ns > ADFT_NOALLOC_MAX_NSPH) {
+        set_error("adft_cart_to_spherical_noalloc: basis of " + std::to_string(ns) + " shells / " + std::to_string(Ns) +
+                  " spherical functions exceeds the static scratch (at most " + std::to_string(ADFT_NOALLOC_MAX_SHELLS) +
+                  " shells and " + std::to_string(ADFT_NOALLOC_MAX_NSPH) + " spherical functions); use adft_cart_to_spherical");
+        return ADFT_ERR_INVALID_ARG;
+    }
+    NoAllocScratch *s = nullptr;
+    adft_status_t rc = noalloc_scratch_ptr(&s);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    noalloc_sph_map_kernel<<<1, 1024, 0, st>>>(p->d_bfoff, ns);
+    CUDA_TRY(cudaGetLastError());
+    dim3 blk(32, 8), grd(((int)Ns + 31) / 32, ((int)Ns + 7) / 8);
+    cart_to_sph_kernel<<<grd, blk, 0, st>>>(M_cart, b->nbf, M_sph, (int)Ns, s->sph_shell, s->sph_m, p->d_bfoff, s->shell_l, &s->tab);
+    CUDA_TRY(cudaGetLastError());
     return ADFT_OK;
 }
