@@ -100,3 +100,24 @@ def test_noalloc_on_a_side_stream_and_argument_errors(api):
     rc = L.adft_cart_to_spherical_noalloc(sp._h, C.c_void_p(sq.data_ptr()), C.c_void_p(sq.data_ptr()), None)
     assert rc == 1 and b"alias" in L.adft_last_error()
     sp.close(); b.close()
+
+
+def test_noalloc_rejects_a_basis_beyond_the_limit(api):
+    """8193 s shells (one more than ADFT_NOALLOC_MAX_SHELLS): refused with ADFT_ERR_INVALID_ARG and a message that names
+    the limit, output untouched; the existing path takes the same basis."""
+    import torch
+    ns = 8193
+    g = int(np.ceil(ns ** (1 / 3)))
+    atoms = np.array([[i, j, k] for i in range(g) for j in range(g) for k in range(g)], float)[:ns] * 3.0
+    shells = np.stack([np.arange(ns), np.zeros(ns), np.ones(ns), np.arange(ns)], 1).astype(np.int32)
+    b = api.Basis(atoms, shells, np.full(ns, 1.3), np.ones(ns))
+    sp = api.ShellPairs(b)
+    M = torch.eye(ns, dtype=torch.float64, device="cuda")
+    out = torch.full((ns, ns), 7.0, dtype=torch.float64, device="cuda")
+    with pytest.raises(api.AdftError) as e:
+        sp.cart_to_spherical_noalloc(M, out)
+    assert e.value.status == 1 and "8192 shells" in str(e.value) and "16384 spherical functions" in str(e.value)
+    torch.cuda.synchronize()
+    assert bool((out == 7.0).all())
+    assert torch.equal(sp.cart_to_spherical(M), M)             # s shells: T = 1
+    sp.close(); b.close()
