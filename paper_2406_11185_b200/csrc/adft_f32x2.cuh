@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(WPB * 32, MINB) jk_kernel_f32x2(const JKParams
         }
         const Segment sg = p.segs[lo];
         const long long r = w - sg.warp_begin;
-        int i = (int)(r / sg.tiles_per_row) * TILE_R + lane / TILE_C;
+        int i = sg.row_begin + (int)(r / sg.tiles_per_row) * TILE_R + lane / TILE_C;
         int j0 = ((int)(r % sg.tiles_per_row) + sg.col_tile_begin) * TILE_C2 + 2 * (lane & (TILE_C - 1));
         int j1 = j0 + 1;
         const int jend = sg.same ? (i + 1) : sg.ket_n;

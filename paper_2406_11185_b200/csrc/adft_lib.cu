@@ -768,6 +768,13 @@ static int prefix_len(const double *q, int n, double qfix, double dmax, double t
 static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax, double tau, std::vector<Segment> &segs,
                             double tau_skip = 0.0, int tile_c = TILE_C)
 {
+    // A (bra sublist, ket sublist) pair keeps the quartets under the staircase Q_ab*Q_cd >= tau/dmax of its rows x columns
+    // matrix (both lists descending in Q).  One rectangle around it would launch two empty tiles for every kept one (cfg 4:
+    // 31% of the launched warps of (ps|ss) held a quartet, and the prologue of the empty ones was a third of that kernel's
+    // instructions), so the rows are cut into bands: a band ends where the row's tile count has fallen to BAND_F of the
+    // band's first row, bands are whole tile rows, and a remainder of fewer than BAND_MIN_TILES tiles stays one band.
+    constexpr double BAND_F = 0.75;
+    constexpr long long BAND_MIN_TILES = 1024;
     segs.clear();
     for (int i1 : p->subl_of_class[X])
         for (int i2 : p->subl_of_class[Y]) {
@@ -776,27 +783,42 @@ static long long plan_class(const adft_shellpairs *p, int X, int Y, double dmax,
             if (s1.n == 0 || s2.n == 0) continue;
             const double *q1 = p->hQ.data() + s1.pair_base, *q2 = p->hQ.data() + s2.pair_base;
             const int rows = prefix_len(q1, s1.n, q2[0], dmax, tau);
-            int cols = prefix_len(q2, s2.n, q1[0], dmax, tau);
             const bool same = (i1 == i2);
-            if (same) cols = std::min(cols, rows);
-            if (rows == 0 || cols == 0) continue;
-            Segment sg{};
-            sg.bra_pair_base = s1.pair_base; sg.bra_prim_base = s1.prim_base; sg.bra_n = s1.n; sg.bra_K = s1.K;
-            sg.ket_pair_base = s2.pair_base; sg.ket_prim_base = s2.prim_base; sg.ket_n = s2.n; sg.ket_K = s2.K;
-            sg.rows = rows; sg.tiles_per_row = (cols + tile_c - 1) / tile_c; sg.same = same ? 1 : 0;
-            if (tau_skip > 0.0) {
-                sg.col_tile_begin = prefix_len(q2, s2.n, q1[rows - 1], dmax, tau_skip) / tile_c;
-                sg.tiles_per_row -= sg.col_tile_begin;
-                if (sg.tiles_per_row <= 0) continue;
+            int r0 = 0;
+            while (r0 < rows) {
+                // kept prefix of the band's first row (the longest of the band); j <= i on the diagonal block
+                int cols = prefix_len(q2, s2.n, q1[r0], dmax, tau);
+                if (cols == 0) break;                                  // cannot happen for r0 < rows; guards the loop
+                const int tiles0 = (std::min(cols, same ? rows : cols) + tile_c - 1) / tile_c;
+                int r1 = rows;
+                if ((long long)((rows - r0 + TILE_R - 1) / TILE_R) * tiles0 >= BAND_MIN_TILES) {
+                    // rows whose prefix still needs at least tmin tiles: q1[r] * q2[(tmin-1)*tile_c] * dmax >= tau
+                    const int tmin = std::max(1, (int)std::ceil(BAND_F * tiles0));
+                    const int cneed = (tmin - 1) * tile_c;             // index of the first column of tile tmin-1
+                    int rb = cneed < s2.n ? prefix_len(q1, rows, q2[cneed], dmax, tau) : r0 + 1;
+                    if (same) rb = std::min(rb, std::max(r0 + TILE_R, (int)((r0 + 1) / BAND_F)));   // diagonal: cols <= i + 1
+                    rb = r0 + std::max(1, (rb - r0) / TILE_R) * TILE_R;                              // whole tile rows
+                    r1 = std::min(rows, rb);
+                }
+                if (same) cols = std::min(cols, r1);
+                Segment sg{};
+                sg.bra_pair_base = s1.pair_base; sg.bra_prim_base = s1.prim_base; sg.bra_n = s1.n; sg.bra_K = s1.K;
+                sg.ket_pair_base = s2.pair_base; sg.ket_prim_base = s2.prim_base; sg.ket_n = s2.n; sg.ket_K = s2.K;
+                sg.row_begin = r0; sg.rows = r1; sg.tiles_per_row = (cols + tile_c - 1) / tile_c; sg.same = same ? 1 : 0;
+                if (tau_skip > 0.0) {
+                    sg.col_tile_begin = prefix_len(q2, s2.n, q1[r1 - 1], dmax, tau_skip) / tile_c;
+                    sg.tiles_per_row -= sg.col_tile_begin;
+                }
+                if (sg.tiles_per_row > 0) segs.push_back(sg);
+                r0 = r1;
             }
-            segs.push_back(sg);
         }
     // heaviest tiles first (per-tile cost ~ K1*K2), so the tail of the launch is made of cheap tiles
     std::stable_sort(segs.begin(), segs.end(), [](const Segment &a, const Segment &b) {
         return (long long)a.bra_K * a.ket_K > (long long)b.bra_K * b.ket_K;
     });
     long long w = 0;
-    for (Segment &s : segs) { s.warp_begin = w; w += (long long)((s.rows + TILE_R - 1) / TILE_R) * s.tiles_per_row; }
+    for (Segment &s : segs) { s.warp_begin = w; w += (long long)((s.rows - s.row_begin + TILE_R - 1) / TILE_R) * s.tiles_per_row; }
     return w;
 }
 

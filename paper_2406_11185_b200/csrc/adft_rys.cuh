@@ -420,7 +420,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p
         }
         const Segment sg = p.segs[lo];
         const long long r = w - sg.warp_begin;
-        const int i_base = (int)(r / sg.tiles_per_row) * TILE_R, j_base = ((int)(r % sg.tiles_per_row) + sg.col_tile_begin) * TILE_C;
+        const int i_base = sg.row_begin + (int)(r / sg.tiles_per_row) * TILE_R, j_base = ((int)(r % sg.tiles_per_row) + sg.col_tile_begin) * TILE_C;
         for (int jj = 0; jj < 32; ++jj) {                       // the 32 quartets of the tile, one after the other
             const int i = i_base + jj / TILE_C, j = j_base + (jj & (TILE_C - 1));
             if (i >= sg.rows) break;
