@@ -202,11 +202,7 @@ __global__ void __launch_bounds__(WPB * 32, MINB) jk_kernel_f32x2(const JKParams
     const int lane = threadIdx.x & 31;
     const long long w = ((long long)blockIdx.x * WPB + (threadIdx.x >> 5)) * p.shard_count + p.shard_rank;
     if (w < p.total_warps) {
-        int lo = 0, hi = p.nsegs - 1;
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (__ldg(&p.segs[mid].warp_begin) <= w) lo = mid; else hi = mid - 1;
-        }
+        const int lo = find_segment(p, w);
         const Segment sg = p.segs[lo];
         const long long r = w - sg.warp_begin;
         int i = sg.row_begin + (int)(r / sg.tiles_per_row) * TILE_R + lane / TILE_C;

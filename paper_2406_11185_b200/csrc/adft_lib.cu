@@ -277,6 +277,8 @@ struct adft_shellpairs {
     // per-build workspaces
     Segment *d_segs = nullptr, *h_segs = nullptr;
     size_t segs_cap = 0;
+    int32_t *d_coarse = nullptr, *h_coarse = nullptr;      // JKParams::coarse of every launch of a build, back to back
+    size_t coarse_cap = 0;
     unsigned long long *d_counters = nullptr, *d_dmax = nullptr, *h_small = nullptr;
     int32_t *d_prim_err = nullptr;     // raised by pair_prim_kernel when a pair's survivor count is not its sublist's K
     cudaEvent_t ev[4 * NQCLASS + 8] = {};      // [0,2N) fp64 class launches, [2N,2N+8) phases, [2N+8,4N+8) fp32 class launches
@@ -433,6 +435,7 @@ static void free_pairs(adft_shellpairs *p)
     cudaFree(p->d_rys); cudaFree(p->d_prim_err); cudaFree(p->d_bfoff); cudaFree(p->d_dsh); cudaFree(p->d_incr);
     cudaFree(p->d_primf); cudaFree(p->d_boysf); cudaFree(p->d_sph); cudaFree(p->d_sph_map);
     if (p->h_segs) cudaFreeHost(p->h_segs);
+    cudaFree(p->d_coarse); if (p->h_coarse) cudaFreeHost(p->h_coarse);
     if (p->h_small) cudaFreeHost(p->h_small);
     if (p->ev_ok) for (auto &e : p->ev) cudaEventDestroy(e);
     delete p;
@@ -919,6 +922,39 @@ extern "C" adft_status_t adft_jk_build_ex(adft_shellpairs_t *p, const double *D,
         }
         if (o) CUDA_TRY(cudaMemcpyAsync(p->d_segs, p->h_segs, o * sizeof(Segment), cudaMemcpyHostToDevice, st));
     }
+    // coarse index of every launch (find_segment): entry k = segment of tile k << COARSE_SHIFT, one entry past the last
+    size_t co_off[NQCLASS] = {}, co_off32[NQCLASS] = {};
+    {
+        auto entries = [](long long w) { return w > 0 ? (size_t)(((w - 1) >> COARSE_SHIFT) + 2) : (size_t)0; };
+        size_t total = 0;
+        for (int qc = 0; qc < NQCLASS; ++qc) {
+            co_off[qc] = total;  total += entries(warps[qc]);
+            co_off32[qc] = total;  total += entries(warps32[qc]);
+        }
+        if (total > p->coarse_cap) {
+            cudaFree(p->d_coarse); if (p->h_coarse) cudaFreeHost(p->h_coarse);
+            p->d_coarse = nullptr; p->h_coarse = nullptr; p->coarse_cap = 0;
+            const size_t cap = total + total / 4 + 64;
+            CUDA_TRY(cudaMalloc((void **)&p->d_coarse, cap * sizeof(int32_t)));
+            CUDA_TRY(cudaMallocHost((void **)&p->h_coarse, cap * sizeof(int32_t)));
+            p->coarse_cap = cap;
+        }
+        auto fill = [&](const std::vector<Segment> &sg, long long w, int32_t *out) {
+            const size_t n = entries(w);
+            int sidx = 0;
+            const int ns = (int)sg.size();
+            for (size_t k = 0; k < n; ++k) {
+                const long long t = (long long)k << COARSE_SHIFT;
+                while (sidx + 1 < ns && sg[sidx + 1].warp_begin <= t) ++sidx;
+                out[k] = sidx;
+            }
+        };
+        for (int qc = 0; qc < NQCLASS; ++qc) {
+            fill(plan[qc], warps[qc], p->h_coarse + co_off[qc]);
+            fill(plan32[qc], warps32[qc], p->h_coarse + co_off32[qc]);
+        }
+        if (total) CUDA_TRY(cudaMemcpyAsync(p->d_coarse, p->h_coarse, total * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    }
     CUDA_TRY(cudaMemsetAsync(p->d_counters, 0, 8 * NQCLASS * sizeof(unsigned long long), st));
     if (J) CUDA_TRY(cudaMemsetAsync(J, 0, n2 * sizeof(double), st));
     if (K) CUDA_TRY(cudaMemsetAsync(K, 0, n2 * sizeof(double), st));
@@ -936,6 +972,7 @@ extern "C" adft_status_t adft_jk_build_ex(adft_shellpairs_t *p, const double *D,
         const bool two = mixed && tau > 0.0 && !ce.use_rys;
         JKParams prm{};
         prm.t = p->tab; prm.segs = p->d_segs + seg_off[qc]; prm.nsegs = (int)plan[qc].size(); prm.total_warps = warps[qc];
+        prm.coarse = p->d_coarse + co_off[qc];
         prm.D = D; prm.J = J; prm.K = K; prm.N = N; prm.tau = two ? tau64 : tau; prm.tau_hi = HUGE_VAL; prm.dmax = dmax;
         prm.boys = p->d_boysp; prm.boys_f = p->d_boysf;
         prm.counters = p->d_counters + 4 * qc; prm.zero = 0;
@@ -955,6 +992,7 @@ extern "C" adft_status_t adft_jk_build_ex(adft_shellpairs_t *p, const double *D,
         if (two && warps32[qc] > 0) {
             // the single-precision band tau <= S < tau64 of this class
             prm.segs = p->d_segs + seg_off32[qc]; prm.nsegs = (int)plan32[qc].size(); prm.total_warps = warps32[qc];
+            prm.coarse = p->d_coarse + co_off32[qc];
             prm.tau = tau; prm.tau_hi = tau64;
             prm.counters = p->d_counters + 4 * NQCLASS + 4 * qc;
             cudaEvent_t *e32 = ev + 2 * NQCLASS + 8;

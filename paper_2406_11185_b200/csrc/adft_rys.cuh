@@ -413,11 +413,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) jk_rys_kernel(const JKParams p
         const long long w = s_tile * p.shard_count + p.shard_rank;
         __syncthreads();
         if (w >= p.total_warps) break;
-        int lo = 0, hi = p.nsegs - 1;
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (__ldg(&p.segs[mid].warp_begin) <= w) lo = mid; else hi = mid - 1;
-        }
+        const int lo = find_segment(p, w);
         const Segment sg = p.segs[lo];
         const long long r = w - sg.warp_begin;
         const int i_base = sg.row_begin + (int)(r / sg.tiles_per_row) * TILE_R, j_base = ((int)(r % sg.tiles_per_row) + sg.col_tile_begin) * TILE_C;
