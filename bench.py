@@ -44,8 +44,8 @@ NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA/clk 
 # {workload: {class: (bytes, source)}}.  A dominant kernel without a capture reports "traffic": null.
 NCU_DRAM_BYTES = {
     "cfg4_300atom_globular_2500bf": {
-        "(dp|pp)": (165.8e9, "profiles/r02_ncu_full_cfg4.md"),
-        "(ps|ss)": (5.51e9, "profiles/r02_ncu_full_cfg4.md"),
+        "(dp|pp)": (166.8e9, "profiles/r02_ncu_full_cfg4.md"),
+        "(ps|ss)": (4.0e9, "profiles/r02_ncu_full_cfg4.md"),
     },
 }
 
